@@ -1,0 +1,142 @@
+/*
+ * nvfp4.h -- C ABI of the B200-native NVFP4 GEMV hot path of arxiv/paper_2606_13233.
+ *
+ * What the library computes (citations are PAPER.md lines; "R<n>" = a reading in DESIGN.md):
+ *   - the format: NVFP4 = E2M1 4-bit elements, one FP8-E4M3 scale per block of 16
+ *     consecutive K, one FP32 global scale per tensor (PAPER.md:344-349 Table 7, :359, :175);
+ *   - the operation: the small-M linear projection  Y[M,N] = X[M,K] * W[N,K]^T
+ *     (Sec. 5 "Y = XW ... at small M", stored here by output channel, R7),
+ *     executed on CUDA cores as a single streaming pass over W (Sec. 5.2);
+ *   - the activation quantizer "Q" that feeds it (Table 3 :209-217).
+ *
+ * Conventions common to every call
+ *   - extern "C"; every function returns an int status (0 = NVFP4_OK, negative = error)
+ *     unless it returns a size or a string.
+ *   - Every pointer marked [device] is CUDA device memory owned by the CALLER and must be
+ *     16-byte aligned; the library never allocates, frees or retains caller memory.
+ *   - Calls are ASYNCHRONOUS: they enqueue kernels on `stream` (a cudaStream_t passed as
+ *     void*, NULL = the legacy default stream) and return; they never synchronise, never
+ *     read device data on the host, and are capturable in a CUDA graph.
+ *   - There is no CPU fallback. On a machine with no usable CUDA device every compute call
+ *     returns NVFP4_ERR_CUDA.
+ *   - Canonical NVFP4 layout of a tensor T[R,K] (the oracle's layout):
+ *       codes  uint8 [R, K/2]  byte j of a row = element k=2j in the LOW nibble, k=2j+1 in
+ *                              the HIGH nibble; a nibble is sign-magnitude E2M1 `s e1 e0 m`
+ *       scales uint8 [R, K/16] E4M3 ("fn"), one per 16 consecutive k, always 0x00..0x7E
+ *       g      float           per-tensor global scale;  value = g * E4M3(scale) * E2M1(code)
+ *   - Shape limits: 1 <= M <= 8, N >= 1, K >= 16 and K % 16 == 0, N*K < 2^40.
+ *     Anything else -> NVFP4_ERR_UNSUPPORTED_SHAPE.
+ *   - Non-finite inputs (NaN/Inf activations): behaviour undefined (documented, untested).
+ */
+#ifndef NVFP4_B200_H_
+#define NVFP4_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NVFP4_ABI_VERSION 1
+
+/* status codes */
+#define NVFP4_OK                      0
+#define NVFP4_ERR_INVALID_ARG        -1   /* NULL pointer, bad enum value, workspace too small */
+#define NVFP4_ERR_UNSUPPORTED_SHAPE  -2   /* M, N, K or a leading dimension outside the limits */
+#define NVFP4_ERR_ALIGNMENT          -3   /* a device pointer is not 16-byte aligned */
+#define NVFP4_ERR_CUDA               -4   /* a CUDA runtime call failed; see nvfp4_last_cuda_error */
+
+/* nvfp4_gemv `mode` */
+#define NVFP4_MODE_W4A4   0   /* x = NVFP4 codes + scales + global scale ("W4A4") */
+#define NVFP4_MODE_W4A16  1   /* x = BF16 activations consumed directly (BASELINE.json configs[3]) */
+
+/* nvfp4_gemv `y_dtype` */
+#define NVFP4_DTYPE_F32   0
+#define NVFP4_DTYPE_BF16  1   /* round-to-nearest-even of the FP32 result */
+
+/* nvfp4_quantize_act `gscale_mode` */
+#define NVFP4_GSCALE_DYNAMIC 0 /* g = max|X| / 2688 over the whole [M,K] call argument; WRITTEN to *gscale (R3) */
+#define NVFP4_GSCALE_STATIC  1 /* *gscale is READ (a calibrated value, the paper's deployed flow) */
+
+/* ABI version == repacked-blob format version. */
+int nvfp4_version(void);
+
+/* Text of the last CUDA error seen by the calling thread's library calls ("" if none).
+ * The pointer stays valid until the next library call on this thread. */
+const char* nvfp4_last_cuda_error(void);
+
+/*
+ * Activation quantizer, steps a1+a2 of SURVEY.md 8(a) (the paper's kernel "Q").
+ * BF16 X[M,K] -> canonical NVFP4.  Bit-exact contract (R1, R2; every op one IEEE binary32
+ * round-to-nearest-even op, in this order):
+ *   g = max|X| / 2688;  per 16-block: t = amax_b / 6; u = t / g; scale = E4M3_RNE(min(u,448));
+ *   d = g * E4M3(scale);  code = sign(x) | E2M1_RNE_sat(|x / d|);  g == 0 or d == 0 -> codes 0.
+ *
+ *   x_bf16   [device] BF16 bits, row m at x_bf16 + m*ldx elements; ldx >= K, ldx % 8 == 0
+ *   codes    [device] out, uint8 [M, K/2] contiguous
+ *   scales   [device] out, uint8 [M, K/16] contiguous (row-major, "non-swizzled")
+ *   gscale   [device] one float; written (DYNAMIC) or read (STATIC)
+ *   workspace/ws_bytes: unused by this version (may be NULL / 0); kept for ABI stability.
+ * One kernel launch (a thread-block cluster does the tensor-wide amax on chip).
+ */
+int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx,
+                       uint8_t* codes, uint8_t* scales, float* gscale, int gscale_mode,
+                       void* workspace, size_t ws_bytes, void* stream);
+
+/*
+ * Offline weight repack, step a0.  The blob holds exactly the information of the canonical
+ * (codes, scales) pair, permuted into the order the GEMV's 128-bit loads consume
+ * (DESIGN.md "Data layout"); rows are padded to a multiple of 64 and K to a multiple of 256
+ * with zero codes / zero scales.  nvfp4_repacked_bytes returns 0 for an unsupported shape.
+ *   codes  [device] uint8 [N, K/2];  scales [device] uint8 [N, K/16];  blob_out [device].
+ * nvfp4_unpack_weight is the exact inverse (blob -> canonical, byte-identical).
+ */
+size_t nvfp4_repacked_bytes(int N, int K);
+int nvfp4_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K,
+                        void* blob_out, void* stream);
+int nvfp4_unpack_weight(const void* blob, int N, int K,
+                        uint8_t* codes_out, uint8_t* scales_out, void* stream);
+
+/*
+ * The GEMV / skinny GEMM, steps a3..a7:  Y[m,n] = sum_k vX[m,k] * vW[n,k],
+ * one pass over the repacked W, each decoded weight reused for all M rows (PAPER.md:161,
+ * challenge C1 :151), products exact inside a 16-block, FP32 accumulation across blocks (R8).
+ *   mode      NVFP4_MODE_W4A4 or NVFP4_MODE_W4A16
+ *   w_blob    [device] from nvfp4_repack_weight for this (N, K)
+ *   w_gscale  [device] one float, the weight tensor's global scale
+ *   x         [device] W4A4: uint8 codes, row m at x + m*ldx BYTES'-worth of elements, i.e.
+ *                      ldx counts code bytes (>= K/2, % 16 == 0);
+ *                      W4A16: BF16 bits, ldx counts elements (>= K, % 8 == 0)
+ *   x_scales  [device] W4A4 only: uint8 [M, K/16] contiguous;  NULL for W4A16
+ *   x_gscale  [device] W4A4 only: one float (e.g. the quantizer's output);  NULL for W4A16
+ *   y         [device] out, row m at y + m*ldy elements of y_dtype; ldy >= N
+ *   workspace [device] at least nvfp4_gemv_workspace_bytes(M,N,K) bytes (0 in this version:
+ *             split-K partials are reduced on chip through cluster shared memory)
+ * Acceptance (BASELINE.json north_star): |y - y_ref| <= 1e-3 * sum_k|w_k x_k| + 1e-6.
+ */
+size_t nvfp4_gemv_workspace_bytes(int M, int N, int K);
+int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K,
+               const void* x, const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx,
+               void* y, int y_dtype, int64_t ldy,
+               void* workspace, size_t ws_bytes, void* stream);
+
+/*
+ * Launch-shape override for sweeps (host-side state, not thread-safe; 0 = use the tuned table):
+ *   ksplit = CTAs of one cluster that split K (1..8), warps = warps per CTA (1..16),
+ *   rows   = weight rows per lane (1 or 2).  Returns NVFP4_ERR_INVALID_ARG if out of range.
+ * nvfp4_gemv_get_config reports what nvfp4_gemv would use for (mode, M, N, K).
+ */
+int nvfp4_gemv_set_config(int ksplit, int warps, int rows);
+int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows);
+
+/*
+ * Glue of the decode chain (step a8, BASELINE.json configs[4]; not part of the paper's kernel):
+ *   h[m,j] = silu(gu[m,j]) * gu[m,I+j],  gu BF16 [M,2I] (row stride 2I), h BF16 [M,I];  I % 8 == 0.
+ */
+int nvfp4_silu_mul(const void* gu_bf16, int M, int I, void* h_bf16, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NVFP4_B200_H_ */
