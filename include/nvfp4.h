@@ -78,7 +78,8 @@ const char* nvfp4_last_cuda_error(void);
  *   scales   [device] out, uint8 [M, K/16] contiguous (row-major, "non-swizzled")
  *   gscale   [device] one float; written (DYNAMIC) or read (STATIC)
  *   workspace/ws_bytes: unused by this version (may be NULL / 0); kept for ABI stability.
- * One kernel launch (a thread-block cluster does the tensor-wide amax on chip).
+ * One kernel launch for M*K <= 524288 (a thread-block cluster does the tensor-wide amax on chip,
+ * X is read once); larger tensors take two launches.
  */
 int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx,
                        uint8_t* codes, uint8_t* scales, float* gscale, int gscale_mode,
@@ -87,8 +88,8 @@ int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx,
 /*
  * Offline weight repack, step a0.  The blob holds exactly the information of the canonical
  * (codes, scales) pair, permuted into the order the GEMV's 128-bit loads consume
- * (DESIGN.md "Data layout"); rows are padded to a multiple of 64 and K to a multiple of 256
- * with zero codes / zero scales.  nvfp4_repacked_bytes returns 0 for an unsupported shape.
+ * (2304-byte cells of 32 rows x 128 k); rows are padded to a
+ * multiple of 32 and K to a multiple of 128 with zero codes / zero scales.  nvfp4_repacked_bytes returns 0 for an unsupported shape.
  *   codes  [device] uint8 [N, K/2];  scales [device] uint8 [N, K/16];  blob_out [device].
  * nvfp4_unpack_weight is the exact inverse (blob -> canonical, byte-identical).
  */
@@ -106,13 +107,17 @@ int nvfp4_unpack_weight(const void* blob, int N, int K,
  *   w_blob    [device] from nvfp4_repack_weight for this (N, K)
  *   w_gscale  [device] one float, the weight tensor's global scale
  *   x         [device] W4A4: uint8 codes, row m at x + m*ldx BYTES'-worth of elements, i.e.
- *                      ldx counts code bytes (>= K/2, % 16 == 0);
+ *                      ldx counts code bytes (>= K/2, % 8 == 0);
  *                      W4A16: BF16 bits, ldx counts elements (>= K, % 8 == 0)
  *   x_scales  [device] W4A4 only: uint8 [M, K/16] contiguous;  NULL for W4A16
  *   x_gscale  [device] W4A4 only: one float (e.g. the quantizer's output);  NULL for W4A16
  *   y         [device] out, row m at y + m*ldy elements of y_dtype; ldy >= N
- *   workspace [device] at least nvfp4_gemv_workspace_bytes(M,N,K) bytes (0 in this version:
- *             split-K partials are reduced on chip through cluster shared memory)
+ *   workspace [device] at least nvfp4_gemv_workspace_bytes(M,N,K) bytes: arrival counters and
+ *             FP32 split-K partials.  It must be ZERO-FILLED once before its first use; every
+ *             call leaves it zero-filled where that matters (the counters), so it can be
+ *             reused by any later call on the same stream, and by CUDA-graph replays.  Calls
+ *             that may run concurrently need separate workspaces.  The size depends on the
+ *             launch shape in effect (query again after nvfp4_gemv_set_config).
  * Acceptance (BASELINE.json north_star): |y - y_ref| <= 1e-3 * sum_k|w_k x_k| + 1e-6.
  */
 size_t nvfp4_gemv_workspace_bytes(int M, int N, int K);
@@ -123,12 +128,14 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
 
 /*
  * Launch-shape override for sweeps (host-side state, not thread-safe; 0 = use the tuned table):
- *   ksplit = CTAs of one cluster that split K (1..8), warps = warps per CTA (1..16),
- *   rows   = weight rows per lane (1 or 2).  Returns NVFP4_ERR_INVALID_ARG if out of range.
+ *   ksplit = number of K ranges (grid.y, 1..64), warps = warps per CTA (1..16),
+ *   rows   = 32-row weight tiles per warp, i.e. weight rows per lane (1, 2 or 4),
+ *   stages = depth of each warp's bulk-copy ring (1..16).
+ * Returns NVFP4_ERR_INVALID_ARG if out of range.
  * nvfp4_gemv_get_config reports what nvfp4_gemv would use for (mode, M, N, K).
  */
-int nvfp4_gemv_set_config(int ksplit, int warps, int rows);
-int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows);
+int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages);
+int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages);
 
 /*
  * Glue of the decode chain (step a8, BASELINE.json configs[4]; not part of the paper's kernel):

@@ -1,0 +1,160 @@
+"""ctypes binding of the C ABI in include/nvfp4.h -- argument marshalling only.
+
+Every function takes torch CUDA tensors (device memory + the current stream are all PyTorch
+is used for), checks nothing the library does not check itself, and raises `Nvfp4Error` on a
+non-zero status.  There is NO fallback: if the shared library is missing, importing this module
+raises, and if no CUDA device is usable every compute call fails with NVFP4_ERR_CUDA.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libnvfp4_b200.so")
+
+MODE_W4A4, MODE_W4A16 = 0, 1
+DTYPE_F32, DTYPE_BF16 = 0, 1
+GSCALE_DYNAMIC, GSCALE_STATIC = 0, 1
+ERR_NAMES = {0: "NVFP4_OK", -1: "NVFP4_ERR_INVALID_ARG", -2: "NVFP4_ERR_UNSUPPORTED_SHAPE",
+             -3: "NVFP4_ERR_ALIGNMENT", -4: "NVFP4_ERR_CUDA"}
+
+# every symbol include/nvfp4.h declares (tests check that the library exports all of them)
+SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp4_repacked_bytes",
+           "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
+           "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul")
+
+
+class Nvfp4Error(RuntimeError):
+    def __init__(self, status, detail=""):
+        self.status = status
+        super().__init__(f"{ERR_NAMES.get(status, status)} {detail}".strip())
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2606_13233_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    c_int, c_i64, c_sz, vp = ctypes.c_int, ctypes.c_int64, ctypes.c_size_t, ctypes.c_void_p
+    lib.nvfp4_version.restype = c_int
+    lib.nvfp4_version.argtypes = []
+    lib.nvfp4_last_cuda_error.restype = ctypes.c_char_p
+    lib.nvfp4_last_cuda_error.argtypes = []
+    lib.nvfp4_quantize_act.restype = c_int
+    lib.nvfp4_quantize_act.argtypes = [vp, c_int, c_int, c_i64, vp, vp, vp, c_int, vp, c_sz, vp]
+    lib.nvfp4_repacked_bytes.restype = c_sz
+    lib.nvfp4_repacked_bytes.argtypes = [c_int, c_int]
+    lib.nvfp4_repack_weight.restype = c_int
+    lib.nvfp4_repack_weight.argtypes = [vp, vp, c_int, c_int, vp, vp]
+    lib.nvfp4_unpack_weight.restype = c_int
+    lib.nvfp4_unpack_weight.argtypes = [vp, c_int, c_int, vp, vp, vp]
+    lib.nvfp4_gemv_workspace_bytes.restype = c_sz
+    lib.nvfp4_gemv_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemv.restype = c_int
+    lib.nvfp4_gemv.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64,
+                               vp, c_sz, vp]
+    lib.nvfp4_gemv_set_config.restype = c_int
+    lib.nvfp4_gemv_set_config.argtypes = [c_int, c_int, c_int, c_int]
+    lib.nvfp4_gemv_get_config.restype = c_int
+    lib.nvfp4_gemv_get_config.argtypes = [c_int, c_int, c_int, c_int] + [ctypes.POINTER(c_int)] * 4
+    lib.nvfp4_silu_mul.restype = c_int
+    lib.nvfp4_silu_mul.argtypes = [vp, c_int, c_int, vp, vp]
+    return lib
+
+
+lib = _load()
+
+
+def _check(status):
+    if status != 0:
+        raise Nvfp4Error(status, lib.nvfp4_last_cuda_error().decode())
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
+
+
+def nvfp4_version() -> int:
+    return lib.nvfp4_version()
+
+
+def nvfp4_quantize_act(x_bf16, codes=None, scales=None, gscale=None, gscale_mode=GSCALE_DYNAMIC):
+    """x_bf16 [M,K] torch.bfloat16 (row stride = x.stride(0)) -> (codes u8 [M,K/2], scales u8 [M,K/16], g f32 [1])."""
+    M, K = x_bf16.shape
+    dev = x_bf16.device
+    if codes is None:
+        codes = torch.empty((M, K // 2), dtype=torch.uint8, device=dev)
+    if scales is None:
+        scales = torch.empty((M, K // 16), dtype=torch.uint8, device=dev)
+    if gscale is None:
+        gscale = torch.zeros(1, dtype=torch.float32, device=dev)
+    _check(lib.nvfp4_quantize_act(_ptr(x_bf16), M, K, x_bf16.stride(0), _ptr(codes), _ptr(scales), _ptr(gscale),
+                                  gscale_mode, None, 0, _stream()))
+    return codes, scales, gscale
+
+
+def nvfp4_repacked_bytes(N, K) -> int:
+    return lib.nvfp4_repacked_bytes(N, K)
+
+
+def nvfp4_repack_weight(codes, scales, blob=None):
+    N, K = codes.shape[0], codes.shape[1] * 2
+    if blob is None:
+        blob = torch.empty(nvfp4_repacked_bytes(N, K), dtype=torch.uint8, device=codes.device)
+    _check(lib.nvfp4_repack_weight(_ptr(codes), _ptr(scales), N, K, _ptr(blob), _stream()))
+    return blob
+
+
+def nvfp4_unpack_weight(blob, N, K):
+    codes = torch.empty((N, K // 2), dtype=torch.uint8, device=blob.device)
+    scales = torch.empty((N, K // 16), dtype=torch.uint8, device=blob.device)
+    _check(lib.nvfp4_unpack_weight(_ptr(blob), N, K, _ptr(codes), _ptr(scales), _stream()))
+    return codes, scales
+
+
+def nvfp4_gemv_workspace_bytes(M, N, K) -> int:
+    return lib.nvfp4_gemv_workspace_bytes(M, N, K)
+
+
+def new_workspace(M, N, K, device="cuda"):
+    """zero-filled workspace (the ABI requires zero fill before first use)."""
+    return torch.zeros(max(16, nvfp4_gemv_workspace_bytes(M, N, K)), dtype=torch.uint8, device=device)
+
+
+def nvfp4_gemv(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, y=None, y_dtype=DTYPE_BF16,
+               workspace=None):
+    """W4A4: x = codes u8 [M,K/2]; W4A16: x = bf16 [M,K].  Returns y [M,N] (f32 or bf16)."""
+    M = x.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x.device)
+    if workspace is None:
+        workspace = new_workspace(M, N, K, x.device)
+    _check(lib.nvfp4_gemv(mode, _ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x), _ptr(x_scales), _ptr(x_gscale), M,
+                          x.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
+    return y
+
+
+def nvfp4_gemv_set_config(ksplit=0, warps=0, rows=0, stages=0):
+    _check(lib.nvfp4_gemv_set_config(ksplit, warps, rows, stages))
+
+
+def nvfp4_gemv_get_config(mode, M, N, K):
+    v = [ctypes.c_int(0) for _ in range(4)]
+    _check(lib.nvfp4_gemv_get_config(mode, M, N, K, *[ctypes.byref(a) for a in v]))
+    return dict(ksplit=v[0].value, warps=v[1].value, rows=v[2].value, stages=v[3].value)
+
+
+def nvfp4_silu_mul(gu_bf16, h=None):
+    M, I2 = gu_bf16.shape
+    I = I2 // 2
+    if h is None:
+        h = torch.empty((M, I), dtype=torch.bfloat16, device=gu_bf16.device)
+    _check(lib.nvfp4_silu_mul(_ptr(gu_bf16), M, I, _ptr(h), _stream()))
+    return h

@@ -1,0 +1,132 @@
+// api.cu -- the C ABI declared in include/nvfp4.h: argument validation, error codes, launch-shape
+// override, and nothing else (every step of the path runs in the kernels).  No CPU fallback.
+#include <stdio.h>
+#include <string.h>
+
+#include "nvfp4_common.cuh"
+#include "nvfp4_internal.h"
+
+using namespace nvfp4;
+
+static thread_local char g_last_err[256] = "";
+static GemvConfig g_override = {0, 0, 0, 0};      // 0 = use the tuned table
+
+static int cuda_fail(cudaError_t e) {
+    snprintf(g_last_err, sizeof(g_last_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    (void)cudaGetLastError();                     // clear the sticky-less error state
+    return NVFP4_ERR_CUDA;
+}
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static bool shape_ok(int M, int N, int K) {
+    return M >= 1 && M <= 8 && N >= 1 && K >= 16 && (K % 16) == 0 && (int64_t)N * K < ((int64_t)1 << 40);
+}
+static GemvConfig effective_config(int mode, int M, int N, int K) {
+    GemvConfig c = gemv_pick_config(mode, M, N, K);
+    if (g_override.ksplit > 0) c.ksplit = g_override.ksplit;
+    if (g_override.warps > 0) c.warps = g_override.warps;
+    if (g_override.rows > 0) c.rows = g_override.rows;
+    if (g_override.stages > 0) c.stages = g_override.stages;
+    const int nch = n_chunks(K);
+    if (c.ksplit > nch) c.ksplit = nch;
+    return c;
+}
+
+extern "C" {
+
+int nvfp4_version(void) { return NVFP4_ABI_VERSION; }
+
+const char* nvfp4_last_cuda_error(void) { return g_last_err; }
+
+int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* codes, uint8_t* scales,
+                       float* gscale, int gscale_mode, void* workspace, size_t ws_bytes, void* stream) {
+    (void)workspace; (void)ws_bytes;
+    g_last_err[0] = 0;
+    if (!x_bf16 || !codes || !scales || !gscale) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(M, 1, K) || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(x_bf16) || !aligned16(codes) || !aligned16(scales) || (reinterpret_cast<uintptr_t>(gscale) & 3u))
+        return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_quantize_act(x_bf16, M, K, ldx, codes, scales, gscale, gscale_mode,
+                                        static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+size_t nvfp4_repacked_bytes(int N, int K) {
+    if (!shape_ok(1, N, K)) return 0;
+    return (size_t)n_tiles(N) * n_chunks(K) * CELL_BYTES;
+}
+
+int nvfp4_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!codes || !scales || !blob_out) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(1, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(codes) || !aligned16(scales) || !aligned16(blob_out)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_repack(codes, scales, N, K, blob_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_unpack_weight(const void* blob, int N, int K, uint8_t* codes_out, uint8_t* scales_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!codes_out || !scales_out || !blob) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(1, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(codes_out) || !aligned16(scales_out) || !aligned16(blob)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_unpack(blob, N, K, codes_out, scales_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+size_t nvfp4_gemv_workspace_bytes(int M, int N, int K) {
+    if (!shape_ok(M, N, K)) return 0;
+    const size_t a = gemv_workspace_bytes_for(M, N, effective_config(NVFP4_MODE_W4A4, M, N, K));
+    const size_t b = gemv_workspace_bytes_for(M, N, effective_config(NVFP4_MODE_W4A16, M, N, K));
+    return a > b ? a : b;
+}
+
+int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K, const void* x,
+               const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
+               int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+    g_last_err[0] = 0;
+    if (mode != NVFP4_MODE_W4A4 && mode != NVFP4_MODE_W4A16) return NVFP4_ERR_INVALID_ARG;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob || !w_gscale || !x || !y) return NVFP4_ERR_INVALID_ARG;
+    if (mode == NVFP4_MODE_W4A4 && (!x_scales || !x_gscale)) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(M, N, K) || ldy < N) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (mode == NVFP4_MODE_W4A4) { if (ldx < K / 2 || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE; }
+    else                         { if (ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE; }
+    if (!aligned16(w_blob) || !aligned16(x) || !aligned16(y) || (workspace && !aligned16(workspace)))
+        return NVFP4_ERR_ALIGNMENT;
+    const GemvConfig cfg = effective_config(mode, M, N, K);
+    const size_t need = gemv_workspace_bytes_for(M, N, cfg);
+    if (cfg.ksplit > 1 && (!workspace || ws_bytes < need)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemv(mode, w_blob, w_gscale, N, K, x, x_scales, x_gscale, M, ldx, y, y_dtype, ldy,
+                                workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages) {
+    if (ksplit < 0 || ksplit > 64 || warps < 0 || warps > 16 || stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
+    if (!(rows == 0 || rows == 1 || rows == 2 || rows == 4)) return NVFP4_ERR_INVALID_ARG;
+    g_override.ksplit = ksplit; g_override.warps = warps; g_override.rows = rows; g_override.stages = stages;
+    return NVFP4_OK;
+}
+
+int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages) {
+    if (mode != NVFP4_MODE_W4A4 && mode != NVFP4_MODE_W4A16) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(M, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    const GemvConfig c = effective_config(mode, M, N, K);
+    if (ksplit) *ksplit = c.ksplit;
+    if (warps) *warps = c.warps;
+    if (rows) *rows = c.rows;
+    if (stages) *stages = c.stages;
+    return NVFP4_OK;
+}
+
+int nvfp4_silu_mul(const void* gu_bf16, int M, int I, void* h_bf16, void* stream) {
+    g_last_err[0] = 0;
+    if (!gu_bf16 || !h_bf16) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || I < 8 || (I % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(gu_bf16) || !aligned16(h_bf16)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_silu_mul(gu_bf16, M, I, h_bf16, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+}  // extern "C"

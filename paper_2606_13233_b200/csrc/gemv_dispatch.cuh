@@ -1,0 +1,46 @@
+// gemv_dispatch.cuh -- runtime (M, R) -> template instantiation.  Included by one .cu per mode so
+// the two families of kernels compile in parallel.
+#pragma once
+#include "gemv_kernel.cuh"
+
+namespace nvfp4 {
+
+template <int MODE, int M, int R>
+static cudaError_t launch_one(const GemvParams& p, dim3 grid, int threads, size_t smem, cudaStream_t st) {
+    static size_t configured = 0;                 // per instantiation; grows monotonically
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(gemv_kernel<MODE, M, R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    gemv_kernel<MODE, M, R><<<grid, threads, smem, st>>>(p);
+    return cudaGetLastError();
+}
+
+template <int MODE, int M>
+static cudaError_t launch_r(const GemvParams& p, int R, dim3 grid, int threads, size_t smem, cudaStream_t st) {
+    switch (R) {
+        case 1: return launch_one<MODE, M, 1>(p, grid, threads, smem, st);
+        case 2: return launch_one<MODE, M, 2>(p, grid, threads, smem, st);
+        case 4: return launch_one<MODE, M, 4>(p, grid, threads, smem, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <int MODE>
+static cudaError_t launch_m(const GemvParams& p, int M, int R, dim3 grid, int threads, size_t smem, cudaStream_t st) {
+    switch (M) {
+        case 1: return launch_r<MODE, 1>(p, R, grid, threads, smem, st);
+        case 2: return launch_r<MODE, 2>(p, R, grid, threads, smem, st);
+        case 3: return launch_r<MODE, 3>(p, R, grid, threads, smem, st);
+        case 4: return launch_r<MODE, 4>(p, R, grid, threads, smem, st);
+        case 5: return launch_r<MODE, 5>(p, R, grid, threads, smem, st);
+        case 6: return launch_r<MODE, 6>(p, R, grid, threads, smem, st);
+        case 7: return launch_r<MODE, 7>(p, R, grid, threads, smem, st);
+        case 8: return launch_r<MODE, 8>(p, R, grid, threads, smem, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace nvfp4

@@ -1,0 +1,326 @@
+// gemv_kernel.cuh -- the weight-streaming NVFP4 GEMV / skinny GEMM (steps a3..a7),
+//   Y[m,n] = sum_k vX[m,k] * vW[n,k]     (CUDA cores only)
+//
+// Design (differs from the paper's FP16 cvt+hfma2 kernel):
+//  * lane <-> weight row.  A warp owns R row tiles (32 rows each) and walks a K range; the
+//    activations of that K range are decoded ONCE per CTA into shared memory and every lane
+//    reads them with warp-uniform (broadcast) LDS, so no cross-lane reduction is ever needed.
+//  * each warp has a PRIVATE ring of S stages filled by 1-D bulk copies (cp.async.bulk ->
+//    UBLKCP, completion on an mbarrier); lane 0 refills a stage as soon as the warp has read
+//    it.  HBM bytes in flight do not depend on registers or on how fast the math runs.
+//  * W4A4 math is integer and exact inside a 16-block: PRMT byte-LUTs turn 4 nibbles into
+//    4 bytes u = 12 + 2*e (two PRMT, one per sign, OR-ed), dp4a against int8 x = 2*e_x with the
+//    accumulator pre-loaded with -12*sum(x); one I2F + FMUL + FFMA per (row, m, block) applies
+//    sW*sX in FP32.  Cross-block accumulation is FP32 (R8).
+//  * W4A16: cvt.rn.f16x2.e2m1x2 -> FP32, FP32 FMA against FP32 copies of the BF16 activations.
+//  * split-K across CTAs (grid.y): FP32 partials in the workspace, summed in fixed order by
+//    the last CTA to arrive (deterministic), which also resets the arrival counter.
+#pragma once
+#include "nvfp4_common.cuh"
+#include "nvfp4_internal.h"
+
+namespace nvfp4 {
+
+struct GemvParams {
+    const uint8_t* blob;
+    const float* w_gscale;
+    const void* x;            // W4A4: codes (uint8, row stride ldx bytes); W4A16: BF16 bits (row stride ldx elements)
+    const uint8_t* x_scales;  // W4A4: [M, K/16]
+    const float* x_gscale;    // W4A4
+    void* y;
+    float* partials;          // [ksplit][M][Npad]
+    unsigned int* counters;   // [grid.x], zero on entry, zero on exit
+    int64_t ldx, ldy;
+    int N, K, ntiles, nch, Npad;
+    int warps, stages, ksplit;
+    int y_bf16;
+};
+
+// shared-memory bytes of activations per 32-k block pair and per m
+constexpr int XBP_W4A4  = 48;    // 32 int8 + {init0, init1, sX0, sX1}
+constexpr int XBP_W4A16 = 128;   // 32 floats
+
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
+}
+__device__ __forceinline__ int dp4a_us(uint32_t a_unsigned, uint32_t b_signed, int c) {
+    int d;
+    asm("dp4a.u32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a_unsigned), "r"(b_signed), "r"(c));
+    return d;
+}
+
+// 8 nibbles (one word, low nibble = lowest k) -> two words of bytes u = 12 + 2*e2m1(code)
+__device__ __forceinline__ void decode_w_u8(uint32_t w, uint32_t& u_lo, uint32_t& u_hi) {
+    const uint32_t t = w ^ 0x88888888u;
+    u_lo = prmt(0x0F0E0D0Cu, 0x18141210u, w) | prmt(0x090A0B0Cu, 0x00040608u, t);
+    u_hi = prmt(0x0F0E0D0Cu, 0x18141210u, w >> 16) | prmt(0x090A0B0Cu, 0x00040608u, t >> 16);
+}
+
+// ---- activation staging: decode the CTA's K range once into shared memory ----------------
+template <int M>
+__device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
+    const int nblk = ncw * 8;                                    // 16-blocks in the range
+    const int kb_total = p.K >> 4;
+    const uint8_t* xc = static_cast<const uint8_t*>(p.x);
+    for (int i = threadIdx.x; i < nblk * M; i += blockDim.x) {
+        const int blk = i / M, m = i - blk * M;
+        const int kb = c0 * 8 + blk;                             // global 16-block index
+        uint2 cw = make_uint2(0u, 0u);
+        float sx = 0.0f;
+        if (kb < kb_total) {
+            cw = __ldg(reinterpret_cast<const uint2*>(xc + (int64_t)m * p.ldx + (int64_t)kb * 8));
+            sx = e4m3_to_float(__ldg(p.x_scales + (int64_t)m * kb_total + kb));
+        }
+        uint32_t out[4];
+        int sum = 0;
+#pragma unroll
+        for (int wi = 0; wi < 2; ++wi) {
+            const uint32_t w = wi ? cw.y : cw.x;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                uint32_t o = 0;
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const uint32_t c = (w >> (16 * h + 4 * b)) & 0xFu;
+                    int v = (int)((0xC8643210u >> (4 * (c & 7u))) & 0xFu);   // 2 * |e2m1|
+                    if (c & 8u) v = -v;
+                    sum += v;
+                    o |= ((uint32_t)v & 0xFFu) << (8 * b);
+                }
+                out[wi * 2 + h] = o;
+            }
+        }
+        const int bp = blk >> 1, half = blk & 1;
+        uint8_t* base = xs + (size_t)(bp * M + m) * XBP_W4A4;
+        *reinterpret_cast<uint4*>(base + half * 16) = make_uint4(out[0], out[1], out[2], out[3]);
+        *reinterpret_cast<int*>(base + 32 + half * 4) = -12 * sum;
+        *reinterpret_cast<float*>(base + 40 + half * 4) = sx;
+    }
+}
+
+template <int M>
+__device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
+    const int nvec = ncw * 16;                                   // 8-element vectors per row in the range
+    const uint16_t* xb = static_cast<const uint16_t*>(p.x);
+    for (int i = threadIdx.x; i < nvec * M; i += blockDim.x) {
+        const int v = i / M, m = i - v * M;
+        const int k0 = c0 * CHUNK_K + v * 8;
+        uint4 raw = make_uint4(0, 0, 0, 0);
+        if (k0 < p.K) raw = __ldg(reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + k0));
+        const int bp = v >> 2, q = v & 3;
+        float* dst = reinterpret_cast<float*>(xs + (size_t)(bp * M + m) * XBP_W4A16) + q * 8;
+        const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            dst[2 * j]     = __uint_as_float(w[j] << 16);
+            dst[2 * j + 1] = __uint_as_float(w[j] & 0xFFFF0000u);
+        }
+    }
+}
+
+template <int MODE, int M, int R>
+__global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int W = p.warps, S = p.stages;
+    constexpr int XBP = (MODE == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16;
+    constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
+
+    // K range of this CTA (whole 128-k chunks)
+    const int c0 = (int)(((int64_t)blockIdx.y * p.nch) / p.ksplit);
+    const int c1 = (int)(((int64_t)(blockIdx.y + 1) * p.nch) / p.ksplit);
+    const int ncw = c1 - c0;
+    const int ncw_max = (p.nch + p.ksplit - 1) / p.ksplit;
+
+    uint8_t* xs = smem;                                                      // activations
+    const size_t xs_bytes = ((size_t)ncw_max * 4 * M * XBP + 127) & ~(size_t)127;
+    uint8_t* ring = smem + xs_bytes + (size_t)warp * S * STAGE_BYTES;        // this warp's stages
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + xs_bytes + (size_t)W * S * STAGE_BYTES) + warp * S;
+
+    const int tile0 = (blockIdx.x * W + warp) * R;
+    int nvalid = p.ntiles - tile0;                                           // valid tiles of this warp
+    nvalid = nvalid < 0 ? 0 : (nvalid > R ? R : nvalid);
+    const uint8_t* wsrc = p.blob + ((int64_t)tile0 * p.nch + c0) * CELL_BYTES;
+    const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
+
+    // ---- prologue: start the weight stream before touching the activations ----
+    if (lane == 0 && nvalid > 0) {
+        for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
+        mbar_fence_init();
+        const int npre = ncw < S ? ncw : S;
+        for (int i = 0; i < npre; ++i) {
+            const uint32_t bar = smem_u32(bars + i);
+            mbar_arrive_expect_tx(bar, (uint32_t)nvalid * CELL_BYTES);
+            for (int r = 0; r < nvalid; ++r)
+                bulk_g2s(smem_u32(ring + (size_t)i * STAGE_BYTES + r * CELL_BYTES),
+                         wsrc + r * tile_stride + (int64_t)i * CELL_BYTES, CELL_BYTES, bar);
+        }
+    }
+    if (MODE == NVFP4_MODE_W4A4) stage_x_w4a4<M>(p, xs, c0, ncw);
+    else                         stage_x_w4a16<M>(p, xs, c0, ncw);
+    __syncthreads();
+
+    float acc[R][M];
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
+
+    if (nvalid > 0) {
+        for (int i = 0; i < ncw; ++i) {
+            const int s = i % S;
+            const uint32_t bar = smem_u32(bars + s);
+            mbar_wait(bar, (uint32_t)(i / S) & 1u);
+            const uint8_t* st = ring + (size_t)s * STAGE_BYTES;
+
+            float sw[R][8];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * 8);
+                const float2 f0 = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
+                const float2 f1 = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
+                const float2 f2 = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
+                const float2 f3 = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
+                sw[r][0] = f0.x; sw[r][1] = f0.y; sw[r][2] = f1.x; sw[r][3] = f1.y;
+                sw[r][4] = f2.x; sw[r][5] = f2.y; sw[r][6] = f3.x; sw[r][7] = f3.y;
+            }
+            const uint8_t* xchunk = xs + (size_t)i * 4 * M * XBP;
+
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {                                  // 32-k block pairs of the chunk
+                uint4 wv[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + j * 512 + lane * 16);
+                const uint8_t* xbp = xchunk + (size_t)j * M * XBP;
+
+                if (MODE == NVFP4_MODE_W4A4) {
+                    uint32_t u[R][8];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        decode_w_u8(wv[r].x, u[r][0], u[r][1]);
+                        decode_w_u8(wv[r].y, u[r][2], u[r][3]);
+                        decode_w_u8(wv[r].z, u[r][4], u[r][5]);
+                        decode_w_u8(wv[r].w, u[r][6], u[r][7]);
+                    }
+#pragma unroll
+                    for (int m = 0; m < M; ++m) {
+                        const uint4 xa = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4);
+                        const uint4 xb = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 16);
+                        const uint4 ax = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 32);
+                        const float sx0 = __uint_as_float(ax.z), sx1 = __uint_as_float(ax.w);
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            int d0 = (int)ax.x, d1 = (int)ax.y;
+                            d0 = dp4a_us(u[r][0], xa.x, d0); d0 = dp4a_us(u[r][1], xa.y, d0);
+                            d0 = dp4a_us(u[r][2], xa.z, d0); d0 = dp4a_us(u[r][3], xa.w, d0);
+                            d1 = dp4a_us(u[r][4], xb.x, d1); d1 = dp4a_us(u[r][5], xb.y, d1);
+                            d1 = dp4a_us(u[r][6], xb.z, d1); d1 = dp4a_us(u[r][7], xb.w, d1);
+                            acc[r][m] = fmaf((float)d0, sw[r][2 * j] * sx0, acc[r][m]);
+                            acc[r][m] = fmaf((float)d1, sw[r][2 * j + 1] * sx1, acc[r][m]);
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const uint32_t ww[4] = {wv[r].x, wv[r].y, wv[r].z, wv[r].w};
+                        float wf[32];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q)
+#pragma unroll
+                            for (int b = 0; b < 4; ++b) {
+                                const uint32_t h2 = e2m1x2_to_f16x2((ww[q] >> (8 * b)) & 0xFFu);
+                                asm("{.reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi;}"
+                                    : "=f"(wf[q * 8 + b * 2]), "=f"(wf[q * 8 + b * 2 + 1]) : "r"(h2));
+                            }
+#pragma unroll
+                        for (int m = 0; m < M; ++m) {
+                            const float4* xf = reinterpret_cast<const float4*>(xbp + m * XBP_W4A16);
+                            float d0a = 0.f, d0b = 0.f, d1a = 0.f, d1b = 0.f;
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) {
+                                const float4 x0 = xf[q], x1 = xf[q + 4];
+                                d0a = fmaf(wf[q * 4 + 0], x0.x, d0a); d0b = fmaf(wf[q * 4 + 1], x0.y, d0b);
+                                d0a = fmaf(wf[q * 4 + 2], x0.z, d0a); d0b = fmaf(wf[q * 4 + 3], x0.w, d0b);
+                                d1a = fmaf(wf[16 + q * 4 + 0], x1.x, d1a); d1b = fmaf(wf[16 + q * 4 + 1], x1.y, d1b);
+                                d1a = fmaf(wf[16 + q * 4 + 2], x1.z, d1a); d1b = fmaf(wf[16 + q * 4 + 3], x1.w, d1b);
+                            }
+                            acc[r][m] = fmaf(d0a + d0b, sw[r][2 * j], acc[r][m]);
+                            acc[r][m] = fmaf(d1a + d1b, sw[r][2 * j + 1], acc[r][m]);
+                        }
+                    }
+                }
+            }
+
+            // every lane has read stage s -> refill it with chunk i+S
+            __syncwarp();
+            if (lane == 0 && i + S < ncw) {
+                mbar_arrive_expect_tx(bar, (uint32_t)nvalid * CELL_BYTES);
+                for (int r = 0; r < nvalid; ++r)
+                    bulk_g2s(smem_u32(ring + (size_t)s * STAGE_BYTES + r * CELL_BYTES),
+                             wsrc + r * tile_stride + (int64_t)(i + S) * CELL_BYTES, CELL_BYTES, bar);
+            }
+        }
+    }
+
+    // ---- epilogue (a6, a7) ----
+    float gs = __ldg(p.w_gscale);
+    if (MODE == NVFP4_MODE_W4A4) gs = (gs * __ldg(p.x_gscale)) * 0.25f;     // ints are 2*e on both sides
+
+    if (p.ksplit == 1) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int n = (tile0 + r) * TILE_ROWS + lane;
+            if (r < nvalid && n < p.N) {
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    const float v = acc[r][m] * gs;
+                    if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
+                    else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
+                }
+            }
+        }
+        return;
+    }
+
+    // split K: publish the partial, the last CTA of this CTA row sums all of them in fixed order
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int n = (tile0 + r) * TILE_ROWS + lane;
+        if (r < nvalid) {
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+                __stcg(p.partials + ((int64_t)blockIdx.y * M + m) * p.Npad + n, acc[r][m]);
+        }
+    }
+    __shared__ unsigned int s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int old = atomicAdd(p.counters + blockIdx.x, 1u);
+        s_last = (old == (unsigned int)p.ksplit - 1u);
+        if (s_last) p.counters[blockIdx.x] = 0u;                          // leave the workspace clean
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int n = (tile0 + r) * TILE_ROWS + lane;
+        if (r < nvalid && n < p.N) {
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                float sum = 0.0f;
+                for (int ks = 0; ks < p.ksplit; ++ks)
+                    sum += __ldcg(p.partials + ((int64_t)ks * M + m) * p.Npad + n);
+                const float v = sum * gs;
+                if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
+                else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
+            }
+        }
+    }
+}
+
+}  // namespace nvfp4

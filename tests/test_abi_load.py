@@ -1,0 +1,80 @@
+"""CPU-side checks of the boundary: the shared library builds/loads, exports every symbol that
+include/nvfp4.h declares, and validates arguments before touching CUDA (no compute without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_13233_b200 import build
+    path = build.build()
+    return ctypes.CDLL(path)
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "nvfp4.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nvfp4_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(lib):
+    syms = declared_symbols()
+    assert len(syms) >= 11
+    for s in syms:
+        assert hasattr(lib, s), f"{s} declared in include/nvfp4.h but not exported"
+
+
+def test_binding_lists_every_symbol():
+    from paper_2606_13233_b200 import binding
+    assert sorted(binding.SYMBOLS) == declared_symbols()
+
+
+def test_version_and_sizes(lib):
+    assert lib.nvfp4_version() == 1
+    lib.nvfp4_repacked_bytes.restype = ctypes.c_size_t
+    # exactly the information of the canonical pair when N % 32 == 0 and K % 128 == 0
+    for N, K in [(2048, 2048), (10240, 5120), (5120, 8192), (51200, 5120), (5120, 25600)]:
+        assert lib.nvfp4_repacked_bytes(N, K) == N * K // 2 + N * K // 16
+    # padding: rows to 32, K to 128
+    assert lib.nvfp4_repacked_bytes(33, 144) == 64 * 256 // 2 + 64 * 256 // 16
+    assert lib.nvfp4_repacked_bytes(0, 128) == 0
+    assert lib.nvfp4_repacked_bytes(32, 24) == 0          # K % 16 != 0
+
+
+def test_argument_validation_without_gpu(lib):
+    vp = ctypes.c_void_p
+    lib.nvfp4_quantize_act.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, vp, vp, vp, ctypes.c_int,
+                                       vp, ctypes.c_size_t, vp]
+    assert lib.nvfp4_quantize_act(None, 1, 64, 64, None, None, None, 0, None, 0, None) == -1
+    fake = vp(0x1000)                                       # never dereferenced: validation fails first
+    assert lib.nvfp4_quantize_act(fake, 9, 64, 64, fake, fake, fake, 0, None, 0, None) == -2   # M > 8
+    assert lib.nvfp4_quantize_act(fake, 1, 40, 40, fake, fake, fake, 0, None, 0, None) == -2   # K % 16
+    assert lib.nvfp4_quantize_act(fake, 1, 64, 64, fake, fake, fake, 7, None, 0, None) == -1   # bad mode
+    assert lib.nvfp4_quantize_act(vp(0x1008), 1, 64, 64, fake, fake, fake, 0, None, 0, None) == -3
+    lib.nvfp4_gemv.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, ctypes.c_int, vp, vp, vp, ctypes.c_int,
+                               ctypes.c_int64, vp, ctypes.c_int, ctypes.c_int64, vp, ctypes.c_size_t, vp]
+    assert lib.nvfp4_gemv(5, fake, fake, 32, 128, fake, fake, fake, 1, 64, fake, 0, 32, None, 0, None) == -1
+    assert lib.nvfp4_gemv(0, fake, fake, 32, 128, fake, None, fake, 1, 64, fake, 0, 32, None, 0, None) == -1
+    assert lib.nvfp4_gemv(0, fake, fake, 32, 128, fake, fake, fake, 0, 64, fake, 0, 32, None, 0, None) == -2
+    assert lib.nvfp4_gemv(0, fake, fake, 32, 128, fake, fake, fake, 1, 64, fake, 0, 16, None, 0, None) == -2  # ldy < N
+
+
+def test_config_table_is_sane(lib):
+    ip = ctypes.POINTER(ctypes.c_int)
+    lib.nvfp4_gemv_get_config.argtypes = [ctypes.c_int] * 4 + [ip] * 4
+    lib.nvfp4_gemv_workspace_bytes.restype = ctypes.c_size_t
+    for N, K in [(2048, 2048), (10240, 5120), (5120, 8192), (51200, 5120), (5120, 25600), (1, 16), (100, 208)]:
+        for M in range(1, 9):
+            for mode in (0, 1):
+                v = [ctypes.c_int(0) for _ in range(4)]
+                assert lib.nvfp4_gemv_get_config(mode, M, N, K, *[ctypes.byref(a) for a in v]) == 0
+                ks, warps, rows, stages = [a.value for a in v]
+                assert 1 <= ks <= (K + 127) // 128 and 1 <= warps <= 16 and rows in (1, 2, 4) and 1 <= stages <= 16
+            assert lib.nvfp4_gemv_workspace_bytes(M, N, K) > 0
+    assert lib.nvfp4_gemv_set_config(0, 0, 3, 0) == -1
+    assert lib.nvfp4_gemv_set_config(0, 0, 0, 0) == 0

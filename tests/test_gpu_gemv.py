@@ -1,0 +1,190 @@
+"""GPU parity: nvfp4_gemv (through the C ABI) vs the float64 oracle, element by element.
+Acceptance (north_star): |y_gpu - y_ref| <= 1e-3 * sum_k|w_k x_k| + 1e-6; BF16 output must be
+bit-identical to RN_bf16 of the same kernel's FP32 output (R9)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import nvfp4_oracle as orc
+from paper_2606_13233_b200 import inputs
+import _gpu_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_13233_b200 import binding
+    yield binding
+    binding.nvfp4_gemv_set_config(0, 0, 0, 0)
+
+
+class Case:
+    """one weight + activation set, quantised by the oracle (W) and by the oracle (X reference)."""
+
+    def __init__(self, B, M, N, K, seed=0, shape_id=0):
+        self.M, self.N, self.K = M, N, K
+        self.wc, self.ws, self.gw = U.oracle_weight(N, K, seed, shape_id)
+        self.xbits = inputs.make_activation_bits(M, K, seed, shape_id)
+        self.xf = orc.bf16_bits_to_f32(self.xbits)
+        self.xc, self.xs, self.gx = orc.quantize(self.xf)
+        self.blob = B.nvfp4_repack_weight(U.dev_u8(self.wc), U.dev_u8(self.ws))
+        self.d_gw = U.dev_f32(self.gw)
+        self.Y44, self.A44 = orc.gemv_w4a4(self.wc, self.ws, self.gw, self.xc, self.xs, self.gx)
+        self.Y416, self.A416 = orc.gemv_w4a16(self.wc, self.ws, self.gw, self.xf)
+
+    def run_w4a4(self, B, dtype, gpu_quant=True):
+        if gpu_quant:      # the path of the configs: X quantised on the GPU, fed straight to the GEMV
+            xc, xs, gx = B.nvfp4_quantize_act(U.dev_bf16_from_bits(self.xbits))
+        else:
+            xc, xs, gx = U.dev_u8(self.xc), U.dev_u8(self.xs), U.dev_f32(self.gx)
+        y = B.nvfp4_gemv(B.MODE_W4A4, self.blob, self.d_gw, self.N, self.K, xc, xs, gx, y_dtype=dtype)
+        torch.cuda.synchronize()
+        return y
+
+    def run_w4a16(self, B, dtype):
+        y = B.nvfp4_gemv(B.MODE_W4A16, self.blob, self.d_gw, self.N, self.K, U.dev_bf16_from_bits(self.xbits),
+                         y_dtype=dtype)
+        torch.cuda.synchronize()
+        return y
+
+
+def check_both_dtypes(B, case, mode, bf16_slack=True):
+    run = case.run_w4a4 if mode == "w4a4" else case.run_w4a16
+    Y, A = (case.Y44, case.A44) if mode == "w4a4" else (case.Y416, case.A416)
+    y32 = run(B, B.DTYPE_F32)
+    U.check_gemv(U.host_y_f64(y32), Y, A, f"{mode} f32 M={case.M} N={case.N} K={case.K}")
+    y16 = run(B, B.DTYPE_BF16)
+    # epilogue pin: BF16 output == RN_bf16(FP32 output of the same kernel), bit for bit
+    want_bits = orc.f32_to_bf16_bits(y32.cpu().numpy())
+    assert np.array_equal(U.host_bf16_bits(y16), want_bits)
+    U.check_gemv(U.host_y_f64(y16), Y, A, f"{mode} bf16 M={case.M} N={case.N} K={case.K}", bf16_slack=bf16_slack)
+
+
+def test_golden_tiny_example(B, golden_dir):
+    """X = worked example B, W = [B ; B reversed]  (tests/golden/quant_example_B.txt)."""
+    G = {}
+    for line in open(os.path.join(golden_dir, "quant_example_B.txt")):
+        line = line.strip()
+        if line and not line.startswith("#"):
+            k, v = line.split(":", 1)
+            G[k.strip()] = v.split()
+    x = np.array([float(v) for v in G["x0"] + G["x1"]], dtype=np.float32)[None, :]
+    w = np.concatenate([x, x[:, ::-1]], axis=0)
+    wc, ws, gw = orc.quantize(w)
+    blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws))
+    xq = B.nvfp4_quantize_act(U.dev_bf16_from_bits(orc.f32_to_bf16_bits(x)))
+    y = B.nvfp4_gemv(B.MODE_W4A4, blob, U.dev_f32(gw), 2, 32, *xq, y_dtype=B.DTYPE_F32)
+    assert U.host_y_f64(y)[0].tolist() == [float(v) for v in G["gemv_w4a4_Y"]]       # exact in FP32 here
+    y = B.nvfp4_gemv(B.MODE_W4A16, blob, U.dev_f32(gw), 2, 32, U.dev_bf16_from_bits(orc.f32_to_bf16_bits(x)),
+                     y_dtype=B.DTYPE_F32)
+    got = U.host_y_f64(y)[0]
+    assert abs(got[1] - float(G["gemv_w4a16_Y1"][0])) <= 1e-3 * float(G["gemv_w4a16_A1"][0]) + 1e-6
+
+
+def test_all_ones_gives_K(B):
+    """all codes +1.0, all scales 1.0, g = 1 -> Y = K exactly (textbook special case)."""
+    for N, K in [(32, 128), (70, 400), (2048, 2048)]:
+        wc = np.full((N, K // 2), 0x22, np.uint8); ws = np.full((N, K // 16), 0x38, np.uint8)
+        blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws))
+        for M in (1, 3, 8):
+            xc = np.full((M, K // 2), 0x22, np.uint8); xs = np.full((M, K // 16), 0x38, np.uint8)
+            y = B.nvfp4_gemv(B.MODE_W4A4, blob, U.dev_f32(1), N, K, U.dev_u8(xc), U.dev_u8(xs), U.dev_f32(1),
+                             y_dtype=B.DTYPE_F32)
+            assert np.all(U.host_y_f64(y) == K)
+            xb = torch.ones((M, K), dtype=torch.bfloat16, device="cuda")
+            y = B.nvfp4_gemv(B.MODE_W4A16, blob, U.dev_f32(1), N, K, xb, y_dtype=B.DTYPE_F32)
+            assert np.all(U.host_y_f64(y) == K)
+
+
+def test_extreme_scales_and_codes_exact(B):
+    """largest magnitudes everywhere (code +-6, scale 448): block dots hit the int bound
+    16*12*12 and FP32 must not overflow; one-hot X row returns a dequantised W column."""
+    N, K = 64, 256
+    rng = np.random.default_rng(3)
+    wc = rng.choice(np.array([0x77, 0xFF, 0x7F, 0xF7], np.uint8), size=(N, K // 2))
+    ws = np.full((N, K // 16), 0x7E, np.uint8)
+    blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws))
+    xc = np.full((2, K // 2), 0x77, np.uint8); xc[1] = 0
+    xc[1, 5] = 0x20                                      # one-hot: k = 11 (high nibble) = +1.0
+    xs = np.full((2, K // 16), 0x7E, np.uint8); xs[1] = 0x38
+    y = B.nvfp4_gemv(B.MODE_W4A4, blob, U.dev_f32(1), N, K, U.dev_u8(xc), U.dev_u8(xs), U.dev_f32(1),
+                     y_dtype=B.DTYPE_F32)
+    Y, A = orc.gemv_w4a4(wc, ws, 1.0, xc, xs, 1.0)
+    got = U.host_y_f64(y)
+    U.check_gemv(got, Y, A, "extreme")
+    assert np.array_equal(got[1], orc.dequantize(wc, ws, 1.0)[:, 11])
+
+
+SMALL = [(1, 32, 128), (2, 100, 208), (3, 257, 400), (4, 96, 1040), (5, 513, 640), (6, 64, 2064),
+         (7, 1000, 384), (8, 300, 1296), (1, 1, 16), (8, 31, 48)]
+
+
+@pytest.mark.parametrize("M,N,K", SMALL)
+def test_small_shapes_both_modes(B, M, N, K):
+    B.nvfp4_gemv_set_config(0, 0, 0, 0)
+    case = Case(B, M, N, K, seed=1, shape_id=M)
+    check_both_dtypes(B, case, "w4a4")
+    check_both_dtypes(B, case, "w4a16")
+    # brute-force dense matmul on the dequantised operands for a few entries (oracle independence)
+    vW = orc.dequantize(case.wc, case.ws, case.gw); vX = orc.dequantize(case.xc, case.xs, case.gx)
+    n = N // 2
+    assert abs(sum(float(vW[n, k]) * float(vX[0, k]) for k in range(K)) - case.Y44[0, n]) <= 1e-9 * case.A44[0, n] + 1e-30
+
+
+@pytest.mark.parametrize("cfg", [(1, 1, 1, 1), (2, 2, 2, 2), (3, 4, 4, 3), (5, 8, 1, 4), (7, 3, 2, 5), (16, 16, 1, 2),
+                                 (4, 1, 4, 8), (64, 2, 2, 3)])
+def test_launch_shapes_agree(B, cfg):
+    """every split-K / rows / warps / stages combination computes the same thing (ragged shapes:
+    N not a multiple of warps*rows*32, K not a multiple of ksplit*128)."""
+    try:
+        B.nvfp4_gemv_set_config(*cfg)
+        for M, N, K in [(1, 200, 1296), (5, 333, 2576), (8, 97, 912)]:
+            case = Case(B, M, N, K, seed=2, shape_id=N)
+            check_both_dtypes(B, case, "w4a4")
+            check_both_dtypes(B, case, "w4a16")
+    finally:
+        B.nvfp4_gemv_set_config(0, 0, 0, 0)
+
+
+def test_workspace_reuse_and_determinism(B):
+    """split-K leaves the workspace clean: repeated calls on one workspace give identical bits."""
+    try:
+        B.nvfp4_gemv_set_config(6, 4, 2, 3)
+        case = Case(B, 4, 500, 2048, seed=4, shape_id=1)
+        ws = B.new_workspace(4, 500, 2048)
+        xc, xs, gx = B.nvfp4_quantize_act(U.dev_bf16_from_bits(case.xbits))
+        ys = [B.nvfp4_gemv(B.MODE_W4A4, case.blob, case.d_gw, 500, 2048, xc, xs, gx, y_dtype=B.DTYPE_F32,
+                           workspace=ws).clone() for _ in range(5)]
+        torch.cuda.synchronize()
+        for y in ys[1:]:
+            assert torch.equal(y, ys[0])
+        U.check_gemv(U.host_y_f64(ys[0]), case.Y44, case.A44, "reuse")
+        assert int(ws[:256].view(torch.int32).abs().sum()) == 0       # counters back to zero
+    finally:
+        B.nvfp4_gemv_set_config(0, 0, 0, 0)
+
+
+def test_config0_single_gemv(B):
+    """BASELINE.json configs[0]: M=1, N=K=2048, seed 0, X quantised on the GPU, FP32 Y."""
+    case = Case(B, 1, 2048, 2048, seed=0, shape_id=0)
+    xq = B.nvfp4_quantize_act(U.dev_bf16_from_bits(case.xbits))
+    torch.cuda.synchronize()
+    assert np.array_equal(U.host_u8(xq[0]), case.xc) and np.array_equal(U.host_u8(xq[1]), case.xs)
+    assert np.float32(xq[2].cpu().numpy()[0]).view(np.uint32) == np.float32(case.gx).view(np.uint32)
+    y = case.run_w4a4(B, B.DTYPE_F32)
+    worst = U.check_gemv(U.host_y_f64(y), case.Y44, case.A44, "config0")
+    assert worst < 0.05        # FP32 cross-block accumulation leaves > 20x margin (R8)
+    # linearity in the global scales: doubling gW doubles Y exactly
+    y2 = B.nvfp4_gemv(B.MODE_W4A4, case.blob, U.dev_f32(2 * case.gw), 2048, 2048, *xq, y_dtype=B.DTYPE_F32)
+    assert torch.equal(y2, 2 * y)
+
+
+@pytest.mark.parametrize("M", [1, 2, 3, 4, 6, 8])
+def test_medium_shape_all_m(B, M):
+    """several CTA rows, several K ranges, the tuned launch shape, every M of configs[2]."""
+    case = Case(B, M, 2048 + 96, 5120, seed=0, shape_id=10 + M)
+    check_both_dtypes(B, case, "w4a4", bf16_slack=False)      # config-like K: tolerance as written
+    check_both_dtypes(B, case, "w4a16", bf16_slack=False)
