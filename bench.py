@@ -1,0 +1,447 @@
+#!/usr/bin/env python
+"""bench.py -- the NVFP4 GEMV hot path on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--m M] [--impl ours|reference] [--sweep]
+
+A "step" is one pass of the whole hot path over one batch: for each of the four Qwen3-32B
+projections (BASELINE.json configs[1]: QKV 10240x5120, O 5120x8192, gate_up 51200x5120,
+down 5120x25600) one `nvfp4_quantize_act` (BF16 -> NVFP4, dynamic global scale) followed by one
+W4A4 `nvfp4_gemv` with BF16 output, at M rows (default 1).  The step is captured in a CUDA graph
+(the paper times with graph replay) and replayed K times between CUDA events.
+L2 is cold for the weights: a step streams 274 MB of weights (> 126 MB L2) and two distinct
+weight sets alternate, so no weight byte is re-read before ~548 MB of other traffic.
+
+`value` = algorithmic bytes of the step (N*K/2 + N*K/16 + activation + output bytes per
+projection, north_star) / time, i.e. achieved GB/s of the whole step including the quantizers.
+`roofline` is for the dominant kernel (the GEMV launches alone, timed in their own graph).
+`e2e` runs the same step through the public Python API from pinned HOST buffers (H2D of the BF16
+activations and D2H of the BF16 outputs inside the timed region).
+`--impl reference` times the CPU oracle (test infrastructure) on a bounded sample.
+`--sweep` additionally prints per-shape / per-M tables (cold and warm L2, W4A16, cuBLAS BF16) as
+extra lines BEFORE the final JSON line, for profiles/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_13233_b200 import inputs  # noqa: E402
+
+SHAPES = inputs.QWEN3_32B_SHAPES
+METRIC = "nvfp4_gemv_achieved_hbm_gbs"
+UNIT = "GB/s"
+WORKLOAD = "configs[1]: Qwen3-32B qkv/o/gate_up/down projections, W4A4, BF16 out, quantize_act + gemv each"
+L2_BYTES = 126 * 1024 * 1024
+
+
+def algorithmic_bytes(M, N, K, with_quant=False):
+    """north_star byte count of one projection: packed W + W scales + activation + output (BF16).
+    GEMV alone reads the quantised activation (codes + scales); with the quantizer in front the
+    activation bytes are the BF16 input of the quantizer plus its NVFP4 output and the re-read."""
+    w = N * K // 2 + N * K // 16
+    xq = M * (K // 2 + K // 16)
+    y = M * N * 2
+    if with_quant:
+        return w + M * K * 2 + 2 * xq + y
+    return w + xq + y
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.stop = [], threading.Event()
+        self.index = index
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.1)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+class Workload:
+    """device state of the step: `copies` distinct weight sets, per-projection activation,
+    NVFP4 activation, output and workspace buffers."""
+
+    def __init__(self, M, copies=2, mode="w4a4", shapes=SHAPES):
+        import torch
+        from paper_2606_13233_b200 import binding as B
+        self.torch, self.B, self.M, self.mode, self.shapes = torch, B, M, mode, shapes
+        self.proj = []
+        for sid, (name, N, K) in enumerate(shapes, start=1):
+            blobs = []
+            for c in range(copies):
+                codes, scales, g = inputs.make_nvfp4_weight_device(N, K, seed=c, shape_id=sid)
+                blobs.append(B.nvfp4_repack_weight(codes, scales))
+                del codes, scales
+            xbits = inputs.make_activation_bits(M, K, seed=0, shape_id=sid)
+            x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
+            self.proj.append(dict(
+                name=name, N=N, K=K, blobs=blobs, gw=torch.tensor([g], dtype=torch.float32, device="cuda"), x=x,
+                x_host=torch.from_numpy(xbits.view(np.int16)).view(torch.bfloat16).pin_memory(),
+                y_host=torch.empty((M, N), dtype=torch.bfloat16).pin_memory(),
+                xc=torch.empty((M, K // 2), dtype=torch.uint8, device="cuda"),
+                xs=torch.empty((M, K // 16), dtype=torch.uint8, device="cuda"),
+                gx=torch.zeros(1, dtype=torch.float32, device="cuda"),
+                y=torch.empty((M, N), dtype=torch.bfloat16, device="cuda"),
+                ws=B.new_workspace(M, N, K)))
+        torch.cuda.synchronize()
+
+    # -- one projection, all on the current stream ------------------------------------------
+    def quantize(self, p):
+        self.B.nvfp4_quantize_act(p["x"], p["xc"], p["xs"], p["gx"])
+
+    def gemv(self, p, copy):
+        B = self.B
+        if self.mode == "w4a4":
+            B.nvfp4_gemv(B.MODE_W4A4, p["blobs"][copy], p["gw"], p["N"], p["K"], p["xc"], p["xs"], p["gx"],
+                         y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
+        else:
+            B.nvfp4_gemv(B.MODE_W4A16, p["blobs"][copy], p["gw"], p["N"], p["K"], p["x"],
+                         y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
+
+    def step(self, copy, quant=True, gemv=True, only=None):
+        n = 0
+        for p in self.proj:
+            if only is not None and p["name"] != only:
+                continue
+            if quant and self.mode == "w4a4":
+                self.quantize(p); n += 1
+            if gemv:
+                self.gemv(p, copy); n += 1
+        return n
+
+    def capture(self, ncopies, **kw):
+        """CUDA graph of `ncopies` consecutive steps (one per weight set); returns (graph, launches)."""
+        torch = self.torch
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            for c in range(ncopies):
+                self.step(c, **kw)            # warm-up outside capture (sets func attributes)
+        torch.cuda.current_stream().wait_stream(s)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        launches = 0
+        with torch.cuda.graph(g):
+            for c in range(ncopies):
+                launches += self.step(c, **kw)
+        return g, launches
+
+    def step_e2e(self, copy):
+        """public-API path from HOST buffers: H2D activations, quantize, gemv, D2H outputs."""
+        for p in self.proj:
+            p["x"].copy_(p["x_host"], non_blocking=True)
+            if self.mode == "w4a4":
+                self.quantize(p)
+            self.gemv(p, copy)
+            p["y_host"].copy_(p["y"], non_blocking=True)
+
+    def bytes_step(self, with_quant=True):
+        return sum(algorithmic_bytes(self.M, p["N"], p["K"], with_quant) for p in self.proj)
+
+
+def time_graph(torch, graph, reps, warmup):
+    """ms per replay: W untimed replays, then `reps` replays between two events, synchronised."""
+    for _ in range(warmup):
+        graph.replay()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        graph.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+# ---- CPU oracle legs (test infrastructure; the ONLY place bench.py touches oracle/) ------------
+def oracle_sample(M, rows_per_shape):
+    """bounded sample of the step for the oracle: the first `rows_per_shape` weight rows of each
+    projection (whole K), the full activations.  Returns (seconds, algorithmic bytes, description)."""
+    from oracle import nvfp4_oracle as orc
+    t_total, bytes_total = 0.0, 0
+    for sid, (name, N, K) in enumerate(SHAPES, start=1):
+        n = min(rows_per_shape, N)
+        rng = np.random.default_rng([0, sid, n])                              # NVFP4-domain weights, same
+        wc = rng.integers(0, 256, size=(n, K // 2), dtype=np.uint8)          # recipe as the device generator
+        ws = rng.integers(0x64, 0x7F, size=(n, K // 16), dtype=np.uint8)
+        gw = np.float32(3.0e-5)
+        xf = inputs.bf16_bits_as_f32(inputs.make_activation_bits(M, K, seed=0, shape_id=sid))
+        t0 = time.perf_counter()
+        xc, xs, gx = orc.quantize(xf)                                        # step a1+a2
+        Y, A = orc.gemv_w4a4(wc, ws, gw, xc, xs, gx)                         # steps a3..a7
+        orc.round_to_bf16(Y)
+        t_total += time.perf_counter() - t0
+        bytes_total += algorithmic_bytes(M, n, K, with_quant=True)
+    return t_total, bytes_total, f"first {rows_per_shape} weight rows of each of the 4 projections, whole K, M={M}"
+
+
+def cpu_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 1) for p in threadpool_info()]
+        return max(n) if n else 1
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    rows = 4096
+    for _ in range(args.warmup):
+        oracle_sample(args.m, 32)
+    ts, nbytes = [], 0
+    for _ in range(args.steps):
+        t, nbytes, desc = oracle_sample(args.m, rows)
+        ts.append(t)
+    t = float(np.mean(ts))
+    val = nbytes / t / 1e9
+    cores = cpu_threads()
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "M": args.m, "sample": desc},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---- our arm -----------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peak, peak_src = measured_peak()
+    M = args.m
+    wl = Workload(M, copies=2)
+    # graphs: the whole step (2 copies per replay), the GEMVs alone, the quantizers alone
+    g_step, n_step = wl.capture(2)
+    g_gemv, n_gemv = wl.capture(2, quant=False)
+    g_q, n_q = wl.capture(2, gemv=False)
+    reps = max(1, (args.steps + 1) // 2)            # one replay = 2 steps
+    wrep = max(2, (args.warmup + 1) // 2)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    with ClockSampler(local) as clk:
+        ms_step = time_graph(torch, g_step, reps, wrep) / 2
+        # keep the sampler running over the kernel-only graphs too (same clocks regime)
+        ms_gemv = time_graph(torch, g_gemv, reps, wrep) / 2
+        ms_q = time_graph(torch, g_q, reps, wrep) / 2
+    barrier()
+    if world > 1:
+        t = torch.tensor([ms_step], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step = float(t.item())
+
+    # end to end through the public API from pinned host buffers
+    for c in range(max(3, args.warmup)):
+        wl.step_e2e(c & 1)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        wl.step_e2e(i & 1)
+    e1.record()
+    barrier()
+    ms_e2e = e0.elapsed_time(e1) / args.steps
+    if world > 1:
+        t = torch.tensor([ms_e2e], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+
+    b_step = wl.bytes_step(with_quant=True)
+    b_gemv = wl.bytes_step(with_quant=False)
+    value = world * b_step / (ms_step * 1e-3) / 1e9
+    ach = b_gemv / (ms_gemv * 1e-3) / 1e9
+    h2d = sum(M * p["K"] * 2 for p in wl.proj)
+    d2h = sum(M * p["N"] * 2 for p in wl.proj)
+
+    per_shape = {}
+    if rank == 0:
+        for p in wl.proj:                               # per-projection cold-L2 numbers (own graphs)
+            g1, _ = wl.capture(2, quant=False, only=p["name"])
+            # a single shape re-read every other launch would be L2-warm for the small ones:
+            # interleave with the full GEMV graph to evict, and subtract it
+            n = 20
+            for _ in range(3):
+                g_gemv.replay(); g1.replay()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(n):
+                g_gemv.replay(); g1.replay()
+            b.record(); torch.cuda.synchronize()
+            us = (a.elapsed_time(b) / n - 2 * ms_gemv) / 2 * 1e3
+            nb = algorithmic_bytes(M, p["N"], p["K"])
+            per_shape[p["name"]] = {"us": round(us, 2), "gbs": round(nb / us / 1e3, 1), "frac": round(nb / us / 1e3 / peak, 3)}
+
+    cpu = None
+    if rank == 0 and not args.no_cpu:
+        t, nb, desc = oracle_sample(M, 8192)
+        cpu = {"value": nb / t / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": desc,
+               "seconds": round(t, 2)}
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "int8 dp4a in-block, f32 across blocks (W4A4 NVFP4 operands)", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "M": M, "l2": "cold: inputs larger than L2 (274 MB weights per step, "
+                       "2 distinct weight sets alternate; L2 = 126 MB)", "timing": "CUDA graph replay, CUDA events",
+                       "multi_gpu": "replicas only"},
+            "us_per_projection": {"step_mean": round(ms_step * 1e3 / 4, 2), "gemv_mean": round(ms_gemv * 1e3 / 4, 2),
+                                  "quantize_mean": round(ms_q * 1e3 / 4, 2), "per_shape_gemv": per_shape},
+            "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone)",
+                         "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": ach / peak,
+                         "traffic": TRAFFIC_BYTES_PER_STEP.get(M)},
+            "e2e": {"value": world * b_step / (ms_e2e * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "cpu_baseline": cpu,
+            "gpu_launches": n_step // 2 * args.steps if args.steps % 2 == 0 else n_step * reps,
+            "clocks": clk.summary(),
+        }
+        if args.sweep:
+            sweep(wl, peak)
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from
+# the committed `ncu --set full` capture (profiles/); None until a capture exists for that M.
+TRAFFIC_BYTES_PER_STEP = {}
+
+
+def sweep(wl0, peak):
+    """per-shape x per-M table: cold L2 (rotating >= 4 distinct weight copies, >= 512 MB), warm L2
+    (same weight replayed), W4A4 and W4A16, and cuBLAS BF16 (torch.matmul) on the same shapes."""
+    import torch
+    from paper_2606_13233_b200 import binding as B
+    del wl0
+    torch.cuda.empty_cache()
+    for sid, (name, N, K) in enumerate(SHAPES, start=1):
+        wbytes = N * K * 9 // 16
+        copies = max(2, -(-4 * L2_BYTES // wbytes))
+        for mode in ("w4a4", "w4a16"):
+            for M in ((1, 2, 3, 4, 6, 8) if mode == "w4a4" else (1, 2, 4, 8)):
+                wl = Workload(M, copies=copies, mode=mode, shapes=((name, N, K),))
+                p = wl.proj[0]
+                cfg = B.nvfp4_gemv_get_config(B.MODE_W4A4 if mode == "w4a4" else B.MODE_W4A16, M, N, K)
+                g_cold, _ = wl.capture(copies, quant=False)
+                g_warm, _ = wl.capture(1, quant=False)
+                g_q, _ = wl.capture(1, gemv=False) if mode == "w4a4" else (None, 0)
+                reps = max(3, 200 // copies)
+                us_cold = time_graph(torch, g_cold, reps, 3) / copies * 1e3
+                us_warm = time_graph(torch, g_warm, 200, 10) * 1e3
+                us_q = time_graph(torch, g_q, 200, 10) * 1e3 if g_q is not None else 0.0
+                nb = algorithmic_bytes(M, N, K) if mode == "w4a4" else wbytes + M * K * 2 + M * N * 2
+                print(json.dumps({"sweep": "nvfp4", "shape": name, "N": N, "K": K, "mode": mode, "M": M, "cfg": cfg,
+                                  "us_cold": round(us_cold, 2), "gbs_cold": round(nb / us_cold / 1e3, 1),
+                                  "frac_cold": round(nb / us_cold / 1e3 / peak, 3), "us_warm": round(us_warm, 2),
+                                  "us_quant": round(us_q, 2), "copies": copies}), flush=True)
+                del wl, g_cold, g_warm, g_q, p
+                torch.cuda.empty_cache()
+        # cuBLAS BF16 on BF16 weights of the same shape (2*N*K bytes): cold rotation and warm
+        ncopy = max(2, -(-4 * L2_BYTES // (2 * N * K)))
+        Ws = [torch.randn(N, K, device="cuda", dtype=torch.bfloat16) * 0.02 for _ in range(ncopy)]
+        for M in (1, 2, 4, 8):
+            x = torch.randn(M, K, device="cuda", dtype=torch.bfloat16)
+            y = torch.empty(M, N, device="cuda", dtype=torch.bfloat16)
+            for w in Ws:
+                torch.matmul(x, w.t(), out=y)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                for w in Ws:
+                    torch.matmul(x, w.t(), out=y)
+            us_cold = time_graph(torch, g, 20, 3) / ncopy * 1e3
+            g2 = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g2):
+                torch.matmul(x, Ws[0].t(), out=y)
+            us_warm = time_graph(torch, g2, 100, 10) * 1e3
+            nb = 2 * N * K + 2 * M * K + 2 * M * N
+            print(json.dumps({"sweep": "cublas_bf16", "shape": name, "N": N, "K": K, "M": M, "us_cold": round(us_cold, 2),
+                              "gbs_cold": round(nb / us_cold / 1e3, 1), "us_warm": round(us_warm, 2)}), flush=True)
+            del g, g2
+        del Ws
+        torch.cuda.empty_cache()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--m", type=int, default=1, help="activation rows M (1..8)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--sweep", action="store_true", help="also print per-shape / per-M / cuBLAS tables")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps == 200 and args.warmup == 20:
+            args.steps, args.warmup = 3, 1
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -75,3 +75,17 @@ def make_activation_bits(M: int, K: int, seed: int = 0, shape_id: int = 0) -> np
     outlier = rng.random(K) < 0.005
     x[:, outlier] *= np.float32(20.0)
     return to_bf16_bits(x)
+
+
+def make_nvfp4_weight_device(N: int, K: int, seed: int = 0, shape_id: int = 0, device="cuda"):
+    """Full-size bench weights drawn directly in the NVFP4 domain ON THE DEVICE (torch RNG):
+    uniform random code bytes, scale bytes uniform in 0x64..0x7E (the range the oracle produces
+    for W ~ N(0, 0.02): DESIGN.md "Input recipe"), and a fixed global scale.  Returns
+    (codes u8 [N,K/2], scales u8 [N,K/16], g float).  Kernel time does not depend on the values;
+    parity at these sizes is tested separately on oracle-quantised weights."""
+    import torch
+    gen = torch.Generator(device=device)
+    gen.manual_seed((int(seed) * 1000003 + int(shape_id)) & 0x7FFFFFFF)
+    codes = torch.randint(0, 256, (N, K // 2), dtype=torch.uint8, device=device, generator=gen)
+    scales = torch.randint(0x64, 0x7F, (N, K // 16), dtype=torch.uint8, device=device, generator=gen)
+    return codes, scales, 3.0e-5
