@@ -425,6 +425,19 @@ def sweep(wl0, peak):
         torch.cuda.empty_cache()
 
 
+def run_profile(args):
+    """no graphs, no events: `steps` plain launches per kernel so that ncu sees ordinary launches."""
+    import torch
+    shapes = tuple(s for s in SHAPES if args.profile_shape in ("all", s[0]))
+    copies = 4 if args.profile_shape != "all" else 2
+    wl = Workload(args.m, copies=copies, mode=args.mode, shapes=shapes)
+    n = 0
+    for i in range(args.warmup + args.steps):
+        n += wl.step(i % copies)
+    torch.cuda.synchronize()
+    print(json.dumps({"profile_shape": args.profile_shape, "M": args.m, "mode": args.mode, "launches": n}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -434,7 +447,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sweep", action="store_true", help="also print per-shape / per-M / cuBLAS tables")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--profile-shape", default=None, help="qkv|o|gate_up|down|all: plain stream launches of "
+                    "quantize_act + gemv on that shape only (for ncu); prints a short JSON line")
+    ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16"])
     args = ap.parse_args()
+    if args.profile_shape:
+        return run_profile(args)
     if args.impl == "reference":
         if args.steps == 200 and args.warmup == 20:
             args.steps, args.warmup = 3, 1

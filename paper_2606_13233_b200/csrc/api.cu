@@ -26,7 +26,7 @@ static GemvConfig effective_config(int mode, int M, int N, int K) {
     if (g_override.warps > 0) c.warps = g_override.warps;
     if (g_override.rows > 0) c.rows = g_override.rows;
     if (g_override.stages > 0) c.stages = g_override.stages;
-    const int nch = n_chunks(K);
+    const int nch = make_layout(N, K, layout_kparts(N, K)).ncells;
     if (c.ksplit > nch) c.ksplit = nch;
     return c;
 }
@@ -53,7 +53,8 @@ int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* c
 
 size_t nvfp4_repacked_bytes(int N, int K) {
     if (!shape_ok(1, N, K)) return 0;
-    return (size_t)n_tiles(N) * n_chunks(K) * CELL_BYTES;
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    return (size_t)L.ntiles * L.ncells * CELL_BYTES;
 }
 
 int nvfp4_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream) {
@@ -76,8 +77,8 @@ int nvfp4_unpack_weight(const void* blob, int N, int K, uint8_t* codes_out, uint
 
 size_t nvfp4_gemv_workspace_bytes(int M, int N, int K) {
     if (!shape_ok(M, N, K)) return 0;
-    const size_t a = gemv_workspace_bytes_for(M, N, effective_config(NVFP4_MODE_W4A4, M, N, K));
-    const size_t b = gemv_workspace_bytes_for(M, N, effective_config(NVFP4_MODE_W4A16, M, N, K));
+    const size_t a = gemv_workspace_bytes_for(M, N, K, effective_config(NVFP4_MODE_W4A4, M, N, K));
+    const size_t b = gemv_workspace_bytes_for(M, N, K, effective_config(NVFP4_MODE_W4A16, M, N, K));
     return a > b ? a : b;
 }
 
@@ -95,7 +96,7 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
     if (!aligned16(w_blob) || !aligned16(x) || !aligned16(y) || (workspace && !aligned16(workspace)))
         return NVFP4_ERR_ALIGNMENT;
     const GemvConfig cfg = effective_config(mode, M, N, K);
-    const size_t need = gemv_workspace_bytes_for(M, N, cfg);
+    const size_t need = gemv_workspace_bytes_for(M, N, K, cfg);
     if (cfg.ksplit > 1 && (!workspace || ws_bytes < need)) return NVFP4_ERR_INVALID_ARG;
     cudaError_t e = launch_gemv(mode, w_blob, w_gscale, N, K, x, x_scales, x_gscale, M, ldx, y, y_dtype, ldy,
                                 workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));

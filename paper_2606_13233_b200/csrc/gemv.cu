@@ -8,11 +8,11 @@ constexpr size_t SMEM_CAP = 227 * 1024;
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-size_t gemv_smem_bytes(int mode, int M, int K, const GemvConfig& c) {
-    const int nch = n_chunks(K);
-    const int ncw_max = (nch + c.ksplit - 1) / c.ksplit;
+size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
     const int xbp = (mode == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16;
-    const size_t xs = align_up((size_t)ncw_max * 4 * M * xbp, 128);
+    const size_t xs = align_up((size_t)ncw_max * 4 * L.kp * M * xbp, 128);
     return xs + (size_t)c.warps * c.stages * c.rows * CELL_BYTES + (size_t)c.warps * c.stages * 8;
 }
 
@@ -20,33 +20,34 @@ size_t gemv_smem_bytes(int mode, int M, int K, const GemvConfig& c) {
 // ("Tuning"); the rule below reproduces them and extrapolates to other shapes.
 GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     GemvConfig c;
-    const int ntiles = n_tiles(N), nch = n_chunks(K);
-    c.rows = (M >= 3 && mode == NVFP4_MODE_W4A4) ? 2 : 1;
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    c.rows = 1;
+    if (mode == NVFP4_MODE_W4A4 && M >= 5 && L.ntiles >= 2 * 8 * NUM_SMS) c.rows = 2;
     c.warps = 8;
     c.stages = 4;
-    if (ntiles < c.rows * c.warps * NUM_SMS / 4) c.rows = 1;
-    const int cta_rows = (ntiles + c.warps * c.rows - 1) / (c.warps * c.rows);
-    const int target = NUM_SMS * 2;
-    int ks = (target + cta_rows / 2) / cta_rows;
-    if (ks * cta_rows > target && ks > 1) --ks;
-    if (ks < 1) ks = 1;
-    if (ks > nch) ks = nch;
-    c.ksplit = ks;
-    // shrink until the CTA fits in shared memory
-    while (gemv_smem_bytes(mode, M, K, c) > SMEM_CAP) {
-        if (c.stages > 2) --c.stages;
-        else if (c.ksplit < nch) ++c.ksplit;
+    c.ksplit = 1;
+    // shrink until the CTA fits in shared memory: K ranges first when the activations dominate
+    while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP / 2) {
+        const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
+        const size_t xs = (size_t)ncw_max * 4 * L.kp * M * ((mode == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16);
+        if (xs > SMEM_CAP / 4 && c.ksplit < L.ncells) ++c.ksplit;
+        else if (c.stages > 2) --c.stages;
+        else if (gemv_smem_bytes(mode, M, N, K, c) <= SMEM_CAP) break;
+        else if (c.ksplit < L.ncells) ++c.ksplit;
         else if (c.warps > 1) c.warps /= 2;
         else break;
     }
     return c;
 }
 
-static size_t counters_bytes(int N) { return align_up((size_t)n_tiles(N) * sizeof(unsigned int), 256); }
+static size_t counters_bytes(int N, int K) {
+    return align_up((size_t)make_layout(N, K, layout_kparts(N, K)).ntiles * sizeof(unsigned int), 256);
+}
 
-size_t gemv_workspace_bytes_for(int M, int N, const GemvConfig& c) {
-    if (c.ksplit <= 1) return counters_bytes(N);
-    return counters_bytes(N) + (size_t)c.ksplit * M * n_tiles(N) * TILE_ROWS * sizeof(float);
+size_t gemv_workspace_bytes_for(int M, int N, int K, const GemvConfig& c) {
+    if (c.ksplit <= 1) return counters_bytes(N, K);
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    return counters_bytes(N, K) + (size_t)c.ksplit * M * L.ntiles * L.rpt * sizeof(float);
 }
 
 cudaError_t launch_gemv_w4a4(const GemvParams& p, int M, int R, dim3 grid, int threads, size_t smem, cudaStream_t st);
@@ -61,14 +62,17 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     p.x = x; p.x_scales = x_scales; p.x_gscale = x_gscale;
     p.y = y;
     p.counters = static_cast<unsigned int*>(workspace);
-    p.partials = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + counters_bytes(N));
+    p.partials = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + counters_bytes(N, K));
     p.ldx = ldx; p.ldy = ldy;
     p.N = N; p.K = K;
-    p.ntiles = n_tiles(N); p.nch = n_chunks(K); p.Npad = p.ntiles * TILE_ROWS;
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    p.ntiles = L.ntiles; p.nch = L.ncells; p.Npad = L.ntiles * L.rpt;
+    p.kp = L.kp; p.kp_shift = 0;
+    while ((1 << p.kp_shift) < L.kp) ++p.kp_shift;
     p.warps = cfg.warps; p.stages = cfg.stages; p.ksplit = cfg.ksplit;
     p.y_bf16 = (y_dtype == NVFP4_DTYPE_BF16);
-    if (cfg.ksplit > 1 && ws_bytes < gemv_workspace_bytes_for(M, N, cfg)) return cudaErrorInvalidValue;
-    const size_t smem = gemv_smem_bytes(mode, M, K, cfg);
+    if (cfg.ksplit > 1 && ws_bytes < gemv_workspace_bytes_for(M, N, K, cfg)) return cudaErrorInvalidValue;
+    const size_t smem = gemv_smem_bytes(mode, M, N, K, cfg);
     if (smem > SMEM_CAP) return cudaErrorInvalidConfiguration;
     dim3 grid((p.ntiles + cfg.warps * cfg.rows - 1) / (cfg.warps * cfg.rows), cfg.ksplit);
     const int threads = cfg.warps * 32;

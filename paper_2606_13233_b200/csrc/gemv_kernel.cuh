@@ -2,9 +2,13 @@
 //   Y[m,n] = sum_k vX[m,k] * vW[n,k]     (CUDA cores only)
 //
 // Design (differs from the paper's FP16 cvt+hfma2 kernel):
-//  * lane <-> weight row.  A warp owns R row tiles (32 rows each) and walks a K range; the
-//    activations of that K range are decoded ONCE per CTA into shared memory and every lane
-//    reads them with warp-uniform (broadcast) LDS, so no cross-lane reduction is ever needed.
+//  * lane <-> (weight row, K part): lane = r*KP + p.  A warp owns R tiles of 32/KP rows and walks
+//    the CTA's K range; the KP lanes of a row take interleaved 32-k vectors and are summed by
+//    log2(KP) warp shuffles ONCE, after the K loop.  KP is a property of the repacked layout
+//    (nvfp4_common.cuh), chosen so that N*KP/32 independent warps fill the GPU: in the tuned
+//    shapes there is no cross-warp and no cross-CTA reduction at all.
+//  * the activations of the K range are decoded ONCE per CTA into shared memory; lanes read
+//    them with LDS.128 (KP distinct addresses per instruction, bank-conflict free).
 //  * each warp has a PRIVATE ring of S stages filled by 1-D bulk copies (cp.async.bulk ->
 //    UBLKCP, completion on an mbarrier); lane 0 refills a stage as soon as the warp has read
 //    it.  HBM bytes in flight do not depend on registers or on how fast the math runs.
@@ -13,8 +17,9 @@
 //    accumulator pre-loaded with -12*sum(x); one I2F + FMUL + FFMA per (row, m, block) applies
 //    sW*sX in FP32.  Cross-block accumulation is FP32 (R8).
 //  * W4A16: cvt.rn.f16x2.e2m1x2 -> FP32, FP32 FMA against FP32 copies of the BF16 activations.
-//  * split-K across CTAs (grid.y): FP32 partials in the workspace, summed in fixed order by
-//    the last CTA to arrive (deterministic), which also resets the arrival counter.
+//  * optional split-K across CTAs (grid.y > 1; only when M*K activations do not fit in shared
+//    memory): FP32 partials in the workspace, summed in fixed order by the last CTA to arrive
+//    (deterministic), which also resets the arrival counter.
 #pragma once
 #include "nvfp4_common.cuh"
 #include "nvfp4_internal.h"
@@ -31,7 +36,8 @@ struct GemvParams {
     float* partials;          // [ksplit][M][Npad]
     unsigned int* counters;   // [grid.x], zero on entry, zero on exit
     int64_t ldx, ldy;
-    int N, K, ntiles, nch, Npad;
+    int N, K, ntiles, nch, Npad;   // tiles of 32/kp rows, cells of 128*kp k, Npad = ntiles * (32/kp)
+    int kp, kp_shift;              // K parts per row inside a warp (power of two) and its log2
     int warps, stages, ksplit;
     int y_bf16;
 };
@@ -61,12 +67,12 @@ __device__ __forceinline__ void decode_w_u8(uint32_t w, uint32_t& u_lo, uint32_t
 // ---- activation staging: decode the CTA's K range once into shared memory ----------------
 template <int M>
 __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
-    const int nblk = ncw * 8;                                    // 16-blocks in the range
+    const int nblk = ncw * 8 * p.kp;                             // 16-blocks in the range
     const int kb_total = p.K >> 4;
     const uint8_t* xc = static_cast<const uint8_t*>(p.x);
     for (int i = threadIdx.x; i < nblk * M; i += blockDim.x) {
         const int blk = i / M, m = i - blk * M;
-        const int kb = c0 * 8 + blk;                             // global 16-block index
+        const int kb = c0 * 8 * p.kp + blk;                      // global 16-block index
         uint2 cw = make_uint2(0u, 0u);
         float sx = 0.0f;
         if (kb < kb_total) {
@@ -102,11 +108,11 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
 
 template <int M>
 __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
-    const int nvec = ncw * 16;                                   // 8-element vectors per row in the range
+    const int nvec = ncw * 16 * p.kp;                            // 8-element vectors per row in the range
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
     for (int i = threadIdx.x; i < nvec * M; i += blockDim.x) {
         const int v = i / M, m = i - v * M;
-        const int k0 = c0 * CHUNK_K + v * 8;
+        const int k0 = c0 * 128 * p.kp + v * 8;
         uint4 raw = make_uint4(0, 0, 0, 0);
         if (k0 < p.K) raw = __ldg(reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + k0));
         const int bp = v >> 2, q = v & 3;
@@ -120,22 +126,88 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
     }
 }
 
+// ---- one 32-k vector (two 16-blocks) of R rows against all M activation rows ------------------
+template <int M, int R>
+__device__ __forceinline__ void block_pair_w4a4(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
+                                                int j, float (&acc)[R][M]) {
+    uint32_t u[R][8];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        decode_w_u8(wv[r].x, u[r][0], u[r][1]);
+        decode_w_u8(wv[r].y, u[r][2], u[r][3]);
+        decode_w_u8(wv[r].z, u[r][4], u[r][5]);
+        decode_w_u8(wv[r].w, u[r][6], u[r][7]);
+    }
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const uint4 xa = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4);
+        const uint4 xb = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 16);
+        const uint4 ax = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 32);
+        const float sx0 = __uint_as_float(ax.z), sx1 = __uint_as_float(ax.w);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int d0 = (int)ax.x, d1 = (int)ax.y;
+            d0 = dp4a_us(u[r][0], xa.x, d0); d0 = dp4a_us(u[r][1], xa.y, d0);
+            d0 = dp4a_us(u[r][2], xa.z, d0); d0 = dp4a_us(u[r][3], xa.w, d0);
+            d1 = dp4a_us(u[r][4], xb.x, d1); d1 = dp4a_us(u[r][5], xb.y, d1);
+            d1 = dp4a_us(u[r][6], xb.z, d1); d1 = dp4a_us(u[r][7], xb.w, d1);
+            acc[r][m] = fmaf((float)d0, sw[r][2 * j] * sx0, acc[r][m]);
+            acc[r][m] = fmaf((float)d1, sw[r][2 * j + 1] * sx1, acc[r][m]);
+        }
+    }
+}
+
+template <int M, int R>
+__device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
+                                                 int j, float (&acc)[R][M]) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const uint32_t ww[4] = {wv[r].x, wv[r].y, wv[r].z, wv[r].w};
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                                      // the two 16-blocks
+            float wf[16];
+#pragma unroll
+            for (int q = 0; q < 2; ++q)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const uint32_t h2 = e2m1x2_to_f16x2((ww[h * 2 + q] >> (8 * b)) & 0xFFu);
+                    asm("{.reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi;}"
+                        : "=f"(wf[q * 8 + b * 2]), "=f"(wf[q * 8 + b * 2 + 1]) : "r"(h2));
+                }
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const float4* xf = reinterpret_cast<const float4*>(xbp + m * XBP_W4A16) + h * 4;
+                float da = 0.f, db = 0.f;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 x = xf[q];
+                    da = fmaf(wf[q * 4 + 0], x.x, da); db = fmaf(wf[q * 4 + 1], x.y, db);
+                    da = fmaf(wf[q * 4 + 2], x.z, da); db = fmaf(wf[q * 4 + 3], x.w, db);
+                }
+                acc[r][m] = fmaf(da + db, sw[r][2 * j + h], acc[r][m]);
+            }
+        }
+    }
+}
+
 template <int MODE, int M, int R>
 __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
+    const int part = lane & (p.kp - 1), rsub = lane >> p.kp_shift;          // lane = rsub*kp + part
+    const int rpt = 32 >> p.kp_shift;
     constexpr int XBP = (MODE == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16;
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
 
-    // K range of this CTA (whole 128-k chunks)
+    // K range of this CTA (whole cells of 128*kp k)
     const int c0 = (int)(((int64_t)blockIdx.y * p.nch) / p.ksplit);
     const int c1 = (int)(((int64_t)(blockIdx.y + 1) * p.nch) / p.ksplit);
     const int ncw = c1 - c0;
     const int ncw_max = (p.nch + p.ksplit - 1) / p.ksplit;
 
     uint8_t* xs = smem;                                                      // activations
-    const size_t xs_bytes = ((size_t)ncw_max * 4 * M * XBP + 127) & ~(size_t)127;
+    const size_t xs_bytes = ((size_t)ncw_max * 4 * p.kp * M * XBP + 127) & ~(size_t)127;
     uint8_t* ring = smem + xs_bytes + (size_t)warp * S * STAGE_BYTES;        // this warp's stages
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + xs_bytes + (size_t)W * S * STAGE_BYTES) + warp * S;
 
@@ -169,10 +241,14 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
         for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
 
     if (nvalid > 0) {
+        int s = 0;
+        uint32_t phase = 0;
+        // this lane's activation records: vector (i*4 + j)*kp + part  ->  stride between j steps = kp records
+        const uint8_t* xlane = xs + (size_t)part * M * XBP;
+        const size_t xstep = (size_t)p.kp * M * XBP;
         for (int i = 0; i < ncw; ++i) {
-            const int s = i % S;
             const uint32_t bar = smem_u32(bars + s);
-            mbar_wait(bar, (uint32_t)(i / S) & 1u);
+            mbar_wait(bar, phase);
             const uint8_t* st = ring + (size_t)s * STAGE_BYTES;
 
             float sw[R][8];
@@ -186,75 +262,20 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
                 sw[r][0] = f0.x; sw[r][1] = f0.y; sw[r][2] = f1.x; sw[r][3] = f1.y;
                 sw[r][4] = f2.x; sw[r][5] = f2.y; sw[r][6] = f3.x; sw[r][7] = f3.y;
             }
-            const uint8_t* xchunk = xs + (size_t)i * 4 * M * XBP;
 
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {                                  // 32-k block pairs of the chunk
+            for (int j = 0; j < 4; ++j) {                                  // four 32-k vectors of this lane
                 uint4 wv[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r)
                     wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + j * 512 + lane * 16);
-                const uint8_t* xbp = xchunk + (size_t)j * M * XBP;
-
-                if (MODE == NVFP4_MODE_W4A4) {
-                    uint32_t u[R][8];
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        decode_w_u8(wv[r].x, u[r][0], u[r][1]);
-                        decode_w_u8(wv[r].y, u[r][2], u[r][3]);
-                        decode_w_u8(wv[r].z, u[r][4], u[r][5]);
-                        decode_w_u8(wv[r].w, u[r][6], u[r][7]);
-                    }
-#pragma unroll
-                    for (int m = 0; m < M; ++m) {
-                        const uint4 xa = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4);
-                        const uint4 xb = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 16);
-                        const uint4 ax = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 32);
-                        const float sx0 = __uint_as_float(ax.z), sx1 = __uint_as_float(ax.w);
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            int d0 = (int)ax.x, d1 = (int)ax.y;
-                            d0 = dp4a_us(u[r][0], xa.x, d0); d0 = dp4a_us(u[r][1], xa.y, d0);
-                            d0 = dp4a_us(u[r][2], xa.z, d0); d0 = dp4a_us(u[r][3], xa.w, d0);
-                            d1 = dp4a_us(u[r][4], xb.x, d1); d1 = dp4a_us(u[r][5], xb.y, d1);
-                            d1 = dp4a_us(u[r][6], xb.z, d1); d1 = dp4a_us(u[r][7], xb.w, d1);
-                            acc[r][m] = fmaf((float)d0, sw[r][2 * j] * sx0, acc[r][m]);
-                            acc[r][m] = fmaf((float)d1, sw[r][2 * j + 1] * sx1, acc[r][m]);
-                        }
-                    }
-                } else {
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        const uint32_t ww[4] = {wv[r].x, wv[r].y, wv[r].z, wv[r].w};
-                        float wf[32];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q)
-#pragma unroll
-                            for (int b = 0; b < 4; ++b) {
-                                const uint32_t h2 = e2m1x2_to_f16x2((ww[q] >> (8 * b)) & 0xFFu);
-                                asm("{.reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi;}"
-                                    : "=f"(wf[q * 8 + b * 2]), "=f"(wf[q * 8 + b * 2 + 1]) : "r"(h2));
-                            }
-#pragma unroll
-                        for (int m = 0; m < M; ++m) {
-                            const float4* xf = reinterpret_cast<const float4*>(xbp + m * XBP_W4A16);
-                            float d0a = 0.f, d0b = 0.f, d1a = 0.f, d1b = 0.f;
-#pragma unroll
-                            for (int q = 0; q < 4; ++q) {
-                                const float4 x0 = xf[q], x1 = xf[q + 4];
-                                d0a = fmaf(wf[q * 4 + 0], x0.x, d0a); d0b = fmaf(wf[q * 4 + 1], x0.y, d0b);
-                                d0a = fmaf(wf[q * 4 + 2], x0.z, d0a); d0b = fmaf(wf[q * 4 + 3], x0.w, d0b);
-                                d1a = fmaf(wf[16 + q * 4 + 0], x1.x, d1a); d1b = fmaf(wf[16 + q * 4 + 1], x1.y, d1b);
-                                d1a = fmaf(wf[16 + q * 4 + 2], x1.z, d1a); d1b = fmaf(wf[16 + q * 4 + 3], x1.w, d1b);
-                            }
-                            acc[r][m] = fmaf(d0a + d0b, sw[r][2 * j], acc[r][m]);
-                            acc[r][m] = fmaf(d1a + d1b, sw[r][2 * j + 1], acc[r][m]);
-                        }
-                    }
-                }
+                const uint8_t* xbp = xlane + (size_t)j * xstep;
+                if (MODE == NVFP4_MODE_W4A4) block_pair_w4a4<M, R>(wv, xbp, sw, j, acc);
+                else                         block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
             }
+            xlane += 4 * xstep;
 
-            // every lane has read stage s -> refill it with chunk i+S
+            // every lane has read stage s -> refill it with cell i+S
             __syncwarp();
             if (lane == 0 && i + S < ncw) {
                 mbar_arrive_expect_tx(bar, (uint32_t)nvalid * CELL_BYTES);
@@ -262,18 +283,28 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
                     bulk_g2s(smem_u32(ring + (size_t)s * STAGE_BYTES + r * CELL_BYTES),
                              wsrc + r * tile_stride + (int64_t)(i + S) * CELL_BYTES, CELL_BYTES, bar);
             }
+            if (++s == S) { s = 0; phase ^= 1u; }
         }
     }
 
-    // ---- epilogue (a6, a7) ----
+    // ---- a6: sum the kp lanes of each row (once) ----
+    for (int off = 1; off < p.kp; off <<= 1) {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int m = 0; m < M; ++m) acc[r][m] += __shfl_xor_sync(0xFFFFFFFFu, acc[r][m], off);
+    }
+    const bool writer = (part == 0);
+
+    // ---- a7: epilogue ----
     float gs = __ldg(p.w_gscale);
     if (MODE == NVFP4_MODE_W4A4) gs = (gs * __ldg(p.x_gscale)) * 0.25f;     // ints are 2*e on both sides
 
     if (p.ksplit == 1) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int n = (tile0 + r) * TILE_ROWS + lane;
-            if (r < nvalid && n < p.N) {
+            const int n = (tile0 + r) * rpt + rsub;
+            if (writer && r < nvalid && n < p.N) {
 #pragma unroll
                 for (int m = 0; m < M; ++m) {
                     const float v = acc[r][m] * gs;
@@ -288,8 +319,8 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
     // split K: publish the partial, the last CTA of this CTA row sums all of them in fixed order
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int n = (tile0 + r) * TILE_ROWS + lane;
-        if (r < nvalid) {
+        const int n = (tile0 + r) * rpt + rsub;
+        if (writer && r < nvalid) {
 #pragma unroll
             for (int m = 0; m < M; ++m)
                 __stcg(p.partials + ((int64_t)blockIdx.y * M + m) * p.Npad + n, acc[r][m]);
@@ -308,8 +339,8 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
     __threadfence();
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int n = (tile0 + r) * TILE_ROWS + lane;
-        if (r < nvalid && n < p.N) {
+        const int n = (tile0 + r) * rpt + rsub;
+        if (writer && r < nvalid && n < p.N) {
 #pragma unroll
             for (int m = 0; m < M; ++m) {
                 float sum = 0.0f;

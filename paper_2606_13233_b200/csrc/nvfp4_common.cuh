@@ -16,18 +16,48 @@
 namespace nvfp4 {
 
 // ---- repacked weight blob geometry -------------------------
-// A "cell" = 32 weight rows (one per lane) x 128 consecutive k:
-//   bytes [0,2048)    codes:  vector j (0..3), lane l -> 16 B = k in [32j, 32j+32) of row l
-//   bytes [2048,2304) scales: lane l -> 8 B = the 8 E4M3 block scales of row l
-// Blob = cells in [tile = n/32][chunk = k/128] order, so one warp streams a contiguous run.
-constexpr int TILE_ROWS   = 32;
-constexpr int CHUNK_K     = 128;
-constexpr int CELL_CODES  = TILE_ROWS * CHUNK_K / 2;   // 2048
-constexpr int CELL_SCALES = TILE_ROWS * CHUNK_K / 16;  // 256
-constexpr int CELL_BYTES  = CELL_CODES + CELL_SCALES;  // 2304
+// A lane of the GEMV owns (row r, K part p): lane = r*KP + p, KP = 2^i K parts per row inside a
+// warp (chosen per weight shape by layout_kparts, so that N*KP/32 independent warp units fill
+// the 148 SMs without any cross-warp or cross-CTA reduction).  A "cell" is what one warp consumes
+// in four 128-bit loads per lane: 32/KP weight rows x 128*KP consecutive k:
+//   bytes [0,2048)    codes:  vector j (0..3), lane (r,p) -> 16 B = the 32 k starting at
+//                             cell_k0 + (j*KP + p)*32 of row tile_row0 + r
+//   bytes [2048,2304) scales: lane (r,p) -> 8 B = the E4M3 scales of those 4 x 2 blocks (j-major)
+// Blob = cells in [tile = n/(32/KP)][cell = k/(128*KP)] order, so one warp streams a contiguous run.
+constexpr int CELL_CODES  = 2048;
+constexpr int CELL_SCALES = 256;
+constexpr int CELL_BYTES  = CELL_CODES + CELL_SCALES;  // 2304 = 0.5625 B per weight
 
-__host__ __device__ inline int n_tiles(int N)  { return (N + TILE_ROWS - 1) / TILE_ROWS; }
-__host__ __device__ inline int n_chunks(int K) { return (K + CHUNK_K - 1) / CHUNK_K; }
+struct Layout {
+    int kp;         // K parts per row inside a warp (1, 2, 4, 8, 16 or 32)
+    int rpt;        // weight rows per tile = 32 / kp
+    int cell_k;     // k per cell = 128 * kp
+    int ntiles;     // ceil(N / rpt)
+    int ncells;     // ceil(K / cell_k)
+};
+
+__host__ __device__ inline Layout make_layout(int N, int K, int kp) {
+    Layout L;
+    L.kp = kp; L.rpt = 32 / kp; L.cell_k = 128 * kp;
+    L.ntiles = (N + L.rpt - 1) / L.rpt;
+    L.ncells = (K + L.cell_k - 1) / L.cell_k;
+    return L;
+}
+
+// K parts for a weight shape: the smallest power of two that yields >= 1184 (= 148 SMs x 8 warps)
+// warp units, among those whose K padding costs at most 3% more than KP = 1 does.
+__host__ __device__ inline int layout_kparts(int N, int K) {
+    const long long pad1 = ((long long)(K + 127) / 128) * 128;
+    int best = 1;
+    for (int kp = 1; kp <= 32; kp *= 2) {
+        const long long ck = 128LL * kp;
+        const long long padk = ((K + ck - 1) / ck) * ck;
+        if (padk * 100 > pad1 * 103) break;
+        best = kp;
+        if ((long long)N * kp >= 1184LL * 32) break;
+    }
+    return best;
+}
 
 // ---- conversions ------------------------------------------------------------------------
 // E4M3 byte pair -> two FP32 (exact): F2FP.E4M3.UNPACK then two f16->f32.

@@ -9,8 +9,8 @@ namespace nvfp4 {
 // launch shape of the GEMV: every field > 0
 struct GemvConfig {
     int warps;    // warps per CTA, each owns `rows` row tiles (32 rows each) -> no cross-warp reduce
-    int rows;     // R: row tiles per warp (1, 2 or 4)
-    int stages;   // depth of each warp's private bulk-copy ring (cells of 128 k)
+    int rows;     // R: row tiles (32/KP rows each) per warp (1, 2 or 4)
+    int stages;   // depth of each warp's private bulk-copy ring (cells of 2304 B per tile)
     int ksplit;   // number of K ranges (grid.y); > 1 -> partials through the workspace
 };
 
@@ -21,8 +21,8 @@ cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, in
 cudaError_t launch_unpack(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st);
 
 GemvConfig gemv_pick_config(int mode, int M, int N, int K);
-size_t gemv_workspace_bytes_for(int M, int N, const GemvConfig& c);
-size_t gemv_smem_bytes(int mode, int M, int K, const GemvConfig& c);
+size_t gemv_workspace_bytes_for(int M, int N, int K, const GemvConfig& c);
+size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c);
 cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, const void* x,
                         const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
                         int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st);

@@ -1,5 +1,6 @@
 // repack.cu -- offline weight repack (step a0) and its exact inverse.  Pure byte permutation:
-// canonical codes[N,K/2] + scales[N,K/16]  <->  blob of 2304-byte cells (nvfp4_common.cuh).
+// canonical codes[N,K/2] + scales[N,K/16]  <->  blob of 2304-byte cells (nvfp4_common.cuh; the
+// K-part count of the layout is a function of (N, K) only).
 // Padding rows (n >= N) and padding k (k >= K) are zero codes / zero scales.
 #include "nvfp4_common.cuh"
 #include "nvfp4_internal.h"
@@ -9,20 +10,21 @@ namespace nvfp4 {
 // one thread per 16-byte code vector of the blob, one per 8-byte scale group
 template <bool TO_BLOB>
 __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes, uint8_t* __restrict__ scales,
-                                                     int N, int K, uint8_t* __restrict__ blob) {
-    const int nch = n_chunks(K);
-    const int64_t ncells = (int64_t)n_tiles(N) * nch;
+                                                     int N, int K, Layout L, uint8_t* __restrict__ blob) {
+    const int64_t ncells = (int64_t)L.ntiles * L.ncells;
     const int64_t nvec = ncells * (128 + 32);               // 128 code vectors + 32 scale groups per cell
     const int64_t rowb = K / 2, rows = K / 16;
     for (int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += (int64_t)gridDim.x * blockDim.x) {
         const int64_t cell = v / 160;
         const int e = (int)(v - cell * 160);
-        const int tile = (int)(cell / nch), chunk = (int)(cell - (int64_t)tile * nch);
+        const int tile = (int)(cell / L.ncells), ci = (int)(cell - (int64_t)tile * L.ncells);
         uint8_t* cellp = blob + cell * CELL_BYTES;
+        const int lane = e & 31;
+        const int n = tile * L.rpt + lane / L.kp, part = lane % L.kp;
         if (e < 128) {
-            const int j = e >> 5, lane = e & 31;
-            const int n = tile * TILE_ROWS + lane;
-            const int64_t b0 = (int64_t)chunk * 64 + j * 16;   // byte offset inside the canonical row
+            const int j = e >> 5;
+            const int64_t k0 = (int64_t)ci * L.cell_k + (int64_t)(j * L.kp + part) * 32;
+            const int64_t b0 = k0 / 2;                          // byte offset inside the canonical row
             uint8_t* bp = cellp + j * 512 + lane * 16;
             for (int i = 0; i < 16; ++i) {
                 const bool valid = (n < N) && (b0 + i < rowb);
@@ -30,35 +32,36 @@ __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes
                 else if (valid) codes[(int64_t)n * rowb + b0 + i] = bp[i];
             }
         } else {
-            const int lane = e - 128;
-            const int n = tile * TILE_ROWS + lane;
-            const int64_t s0 = (int64_t)chunk * 8;
             uint8_t* sp = cellp + CELL_CODES + lane * 8;
             for (int i = 0; i < 8; ++i) {
-                const bool valid = (n < N) && (s0 + i < rows);
-                if (TO_BLOB) sp[i] = valid ? scales[(int64_t)n * rows + s0 + i] : (uint8_t)0;
-                else if (valid) scales[(int64_t)n * rows + s0 + i] = sp[i];
+                const int j = i >> 1;
+                const int64_t s0 = ((int64_t)ci * L.cell_k + (int64_t)(j * L.kp + part) * 32) / 16 + (i & 1);
+                const bool valid = (n < N) && (s0 < rows);
+                if (TO_BLOB) sp[i] = valid ? scales[(int64_t)n * rows + s0] : (uint8_t)0;
+                else if (valid) scales[(int64_t)n * rows + s0] = sp[i];
             }
         }
     }
 }
 
-static int repack_grid(int N, int K) {
-    const int64_t nvec = (int64_t)n_tiles(N) * n_chunks(K) * 160;
+static int repack_grid(const Layout& L) {
+    const int64_t nvec = (int64_t)L.ntiles * L.ncells * 160;
     int64_t g = (nvec + 255) / 256;
     if (g > 148 * 32) g = 148 * 32;
     return (int)g;
 }
 
 cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob, cudaStream_t st) {
-    repack_kernel<true><<<repack_grid(N, K), 256, 0, st>>>(const_cast<uint8_t*>(codes), const_cast<uint8_t*>(scales),
-                                                           N, K, static_cast<uint8_t*>(blob));
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    repack_kernel<true><<<repack_grid(L), 256, 0, st>>>(const_cast<uint8_t*>(codes), const_cast<uint8_t*>(scales),
+                                                        N, K, L, static_cast<uint8_t*>(blob));
     return cudaGetLastError();
 }
 
 cudaError_t launch_unpack(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st) {
-    repack_kernel<false><<<repack_grid(N, K), 256, 0, st>>>(codes, scales, N, K,
-                                                            static_cast<uint8_t*>(const_cast<void*>(blob)));
+    const Layout L = make_layout(N, K, layout_kparts(N, K));
+    repack_kernel<false><<<repack_grid(L), 256, 0, st>>>(codes, scales, N, K, L,
+                                                         static_cast<uint8_t*>(const_cast<void*>(blob)));
     return cudaGetLastError();
 }
 

@@ -40,8 +40,11 @@ def test_version_and_sizes(lib):
     # exactly the information of the canonical pair when N % 32 == 0 and K % 128 == 0
     for N, K in [(2048, 2048), (10240, 5120), (5120, 8192), (51200, 5120), (5120, 25600)]:
         assert lib.nvfp4_repacked_bytes(N, K) == N * K // 2 + N * K // 16
-    # padding: rows to 32, K to 128
-    assert lib.nvfp4_repacked_bytes(33, 144) == 64 * 256 // 2 + 64 * 256 // 16
+    # ragged shapes: whole 2304-byte cells, never less than the canonical information, bounded padding
+    for N, K in [(33, 144), (100, 208), (1, 16), (1000, 2576)]:
+        b = lib.nvfp4_repacked_bytes(N, K)
+        assert b % 2304 == 0 and b >= N * K * 9 // 16
+        assert b <= (N + 31) * ((K + 127) // 128 * 128 * 1.04) * 9 / 16 + 2304
     assert lib.nvfp4_repacked_bytes(0, 128) == 0
     assert lib.nvfp4_repacked_bytes(32, 24) == 0          # K % 16 != 0
 
