@@ -1,4 +1,5 @@
 // gemv.cu -- host side of the GEMV: launch-shape table, workspace layout, template dispatch.
+#include <stdlib.h>
 #include "gemv_kernel.cuh"
 
 namespace nvfp4 {
@@ -23,9 +24,13 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     const Layout L = make_layout(N, K, layout_kparts(N, K));
     c.rows = 1;
     if (mode == NVFP4_MODE_W4A4 && M >= 5 && L.ntiles >= 2 * 8 * NUM_SMS) c.rows = 2;
-    c.warps = 8;
     c.stages = 4;
     c.ksplit = 1;
+    {   // one warp per unit when the units fit one wave of <= 16 warps per SM
+        const int units = (L.ntiles + c.rows - 1) / c.rows;
+        int w = (units + NUM_SMS - 1) / NUM_SMS;
+        c.warps = w < 4 ? 4 : (w > 16 ? 16 : w);
+    }
     // shrink until the CTA fits in shared memory: K ranges first when the activations dominate
     while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP / 2) {
         const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
@@ -71,10 +76,17 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     while ((1 << p.kp_shift) < L.kp) ++p.kp_shift;
     p.warps = cfg.warps; p.stages = cfg.stages; p.ksplit = cfg.ksplit;
     p.y_bf16 = (y_dtype == NVFP4_DTYPE_BF16);
+    p.zero = 0;
+    { const char* e = getenv("NVFP4_DBG"); p.dbg = e ? atoi(e) : 0; }
     if (cfg.ksplit > 1 && ws_bytes < gemv_workspace_bytes_for(M, N, K, cfg)) return cudaErrorInvalidValue;
     const size_t smem = gemv_smem_bytes(mode, M, N, K, cfg);
     if (smem > SMEM_CAP) return cudaErrorInvalidConfiguration;
-    dim3 grid((p.ntiles + cfg.warps * cfg.rows - 1) / (cfg.warps * cfg.rows), cfg.ksplit);
+    p.units = (p.ntiles + cfg.rows - 1) / cfg.rows;
+    int ctas = NUM_SMS / cfg.ksplit;                      // about one CTA per SM over all K ranges
+    { const char* e = getenv("NVFP4_CTAS"); if (e) ctas = atoi(e); }
+    if (ctas < 1) ctas = 1;
+    if (ctas > p.units) ctas = p.units;
+    dim3 grid(ctas, cfg.ksplit);
     const int threads = cfg.warps * 32;
     if (mode == NVFP4_MODE_W4A4) return launch_gemv_w4a4(p, M, cfg.rows, grid, threads, smem, st);
     return launch_gemv_w4a16(p, M, cfg.rows, grid, threads, smem, st);

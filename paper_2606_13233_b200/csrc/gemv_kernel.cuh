@@ -34,12 +34,15 @@ struct GemvParams {
     const float* x_gscale;    // W4A4
     void* y;
     float* partials;          // [ksplit][M][Npad]
-    unsigned int* counters;   // [grid.x], zero on entry, zero on exit
+    unsigned int* counters;   // [units], zero on entry, zero on exit
     int64_t ldx, ldy;
     int N, K, ntiles, nch, Npad;   // tiles of 32/kp rows, cells of 128*kp k, Npad = ntiles * (32/kp)
     int kp, kp_shift;              // K parts per row inside a warp (power of two) and its log2
     int warps, stages, ksplit;
+    int units;                     // ceil(ntiles / R): work items shared by the gridDim.x CTAs of a K range
     int y_bf16;
+    int zero;                      // always 0 (see make_wlut)
+    int dbg;
 };
 
 // shared-memory bytes of activations per 32-k block pair and per m
@@ -57,52 +60,82 @@ __device__ __forceinline__ int dp4a_us(uint32_t a_unsigned, uint32_t b_signed, i
     return d;
 }
 
+// byte LUTs of u = 12 + 2*e2m1: positive codes (index = low 3 bits) and negative codes.  PRMT
+// with selector bit 3 set replicates the MSB (0) of the selected byte, i.e. yields 0x00, so the
+// "wrong sign" half of each lookup vanishes and the two lookups can be OR-ed.
+struct WLut { uint32_t p_lo, p_hi, n_lo, n_hi; };
+__device__ __forceinline__ WLut make_wlut(uint32_t zero) {
+    // The constants are OR-ed with a per-thread value the compiler cannot prove to be 0, so it treats
+    // them as ordinary per-thread registers: otherwise it keeps them in UNIFORM registers and
+    // copies them back with one IMAD.U32 per PRMT (54 extra instructions per 128 weights).
+    WLut l;
+    const uint32_t z = threadIdx.x * zero;     // zero is a kernel parameter that is always 0
+    asm volatile("or.b32 %0, %4, 0x0F0E0D0C; or.b32 %1, %4, 0x18141210; or.b32 %2, %4, 0x090A0B0C; or.b32 %3, %4, 0x00040608;"
+                 : "=r"(l.p_lo), "=r"(l.p_hi), "=r"(l.n_lo), "=r"(l.n_hi) : "r"(z));
+    return l;
+}
 // 8 nibbles (one word, low nibble = lowest k) -> two words of bytes u = 12 + 2*e2m1(code)
-__device__ __forceinline__ void decode_w_u8(uint32_t w, uint32_t& u_lo, uint32_t& u_hi) {
+__device__ __forceinline__ void decode_w_u8(const WLut& l, uint32_t w, uint32_t& u_lo, uint32_t& u_hi) {
     const uint32_t t = w ^ 0x88888888u;
-    u_lo = prmt(0x0F0E0D0Cu, 0x18141210u, w) | prmt(0x090A0B0Cu, 0x00040608u, t);
-    u_hi = prmt(0x0F0E0D0Cu, 0x18141210u, w >> 16) | prmt(0x090A0B0Cu, 0x00040608u, t >> 16);
+    u_lo = prmt(l.p_lo, l.p_hi, w) | prmt(l.n_lo, l.n_hi, t);
+    u_hi = prmt(l.p_lo, l.p_hi, w >> 16) | prmt(l.n_lo, l.n_hi, t >> 16);
 }
 
 // ---- activation staging: decode the CTA's K range once into shared memory ----------------
+// Loads are issued in batches of STAGE_BATCH per thread before any of them is used, so the L2
+// latency is paid once per batch, not once per block.
+constexpr int STAGE_BATCH = 8;
+
+__device__ __forceinline__ void decode_x_block(uint2 cw, float sx, uint8_t* base, int half) {
+    // nibble -> signed int8 x = 2*e2m1: magnitude LUT through PRMT once per sign, per-byte subtract
+    uint32_t out[4];
+    int sum = 0;
+#pragma unroll
+    for (int wi = 0; wi < 2; ++wi) {
+        const uint32_t w = wi ? cw.y : cw.x;
+        const uint32_t t = w ^ 0x88888888u;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint32_t pos = prmt(0x03020100u, 0x0C080604u, w >> (16 * h));   // negative codes -> 0
+            const uint32_t neg = prmt(0x03020100u, 0x0C080604u, t >> (16 * h));   // positive codes -> 0
+            out[wi * 2 + h] = __vsub4(pos, neg);
+            sum += (int)__dp4a(pos, 0x01010101u, 0u) - (int)__dp4a(neg, 0x01010101u, 0u);
+        }
+    }
+    *reinterpret_cast<uint4*>(base + half * 16) = make_uint4(out[0], out[1], out[2], out[3]);
+    *reinterpret_cast<int*>(base + 32 + half * 4) = -12 * sum;
+    *reinterpret_cast<float*>(base + 40 + half * 4) = sx;
+}
+
 template <int M>
 __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
     const int nblk = ncw * 8 * p.kp;                             // 16-blocks in the range
     const int kb_total = p.K >> 4;
+    const int kb0 = c0 * 8 * p.kp;
     const uint8_t* xc = static_cast<const uint8_t*>(p.x);
-    for (int i = threadIdx.x; i < nblk * M; i += blockDim.x) {
-        const int blk = i / M, m = i - blk * M;
-        const int kb = c0 * 8 * p.kp + blk;                      // global 16-block index
-        uint2 cw = make_uint2(0u, 0u);
-        float sx = 0.0f;
-        if (kb < kb_total) {
-            cw = __ldg(reinterpret_cast<const uint2*>(xc + (int64_t)m * p.ldx + (int64_t)kb * 8));
-            sx = e4m3_to_float(__ldg(p.x_scales + (int64_t)m * kb_total + kb));
-        }
-        uint32_t out[4];
-        int sum = 0;
+    const int total = nblk * M;
+    for (int i0 = threadIdx.x; i0 < total; i0 += blockDim.x * STAGE_BATCH) {
+        uint2 cw[STAGE_BATCH];
+        uint32_t sb[STAGE_BATCH];
 #pragma unroll
-        for (int wi = 0; wi < 2; ++wi) {
-            const uint32_t w = wi ? cw.y : cw.x;
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                uint32_t o = 0;
-#pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    const uint32_t c = (w >> (16 * h + 4 * b)) & 0xFu;
-                    int v = (int)((0xC8643210u >> (4 * (c & 7u))) & 0xFu);   // 2 * |e2m1|
-                    if (c & 8u) v = -v;
-                    sum += v;
-                    o |= ((uint32_t)v & 0xFFu) << (8 * b);
-                }
-                out[wi * 2 + h] = o;
+        for (int t = 0; t < STAGE_BATCH; ++t) {
+            const int i = i0 + t * blockDim.x;
+            const int m = (M == 1) ? 0 : i / nblk, blk = (M == 1) ? i : i - m * nblk;
+            cw[t] = make_uint2(0u, 0u);
+            sb[t] = 0;
+            if (i < total && kb0 + blk < kb_total) {
+                cw[t] = __ldg(reinterpret_cast<const uint2*>(xc + (int64_t)m * p.ldx + (int64_t)(kb0 + blk) * 8));
+                sb[t] = __ldg(p.x_scales + (int64_t)m * kb_total + kb0 + blk);
             }
         }
-        const int bp = blk >> 1, half = blk & 1;
-        uint8_t* base = xs + (size_t)(bp * M + m) * XBP_W4A4;
-        *reinterpret_cast<uint4*>(base + half * 16) = make_uint4(out[0], out[1], out[2], out[3]);
-        *reinterpret_cast<int*>(base + 32 + half * 4) = -12 * sum;
-        *reinterpret_cast<float*>(base + 40 + half * 4) = sx;
+#pragma unroll
+        for (int t = 0; t < STAGE_BATCH; ++t) {
+            const int i = i0 + t * blockDim.x;
+            if (i < total) {
+                const int m = (M == 1) ? 0 : i / nblk, blk = (M == 1) ? i : i - m * nblk;
+                decode_x_block(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)((blk >> 1) * M + m) * XBP_W4A4, blk & 1);
+            }
+        }
     }
 }
 
@@ -110,33 +143,48 @@ template <int M>
 __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
     const int nvec = ncw * 16 * p.kp;                            // 8-element vectors per row in the range
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
-    for (int i = threadIdx.x; i < nvec * M; i += blockDim.x) {
-        const int v = i / M, m = i - v * M;
-        const int k0 = c0 * 128 * p.kp + v * 8;
-        uint4 raw = make_uint4(0, 0, 0, 0);
-        if (k0 < p.K) raw = __ldg(reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + k0));
-        const int bp = v >> 2, q = v & 3;
-        float* dst = reinterpret_cast<float*>(xs + (size_t)(bp * M + m) * XBP_W4A16) + q * 8;
-        const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+    const int total = nvec * M;
+    const int k_base = c0 * 128 * p.kp;
+    for (int i0 = threadIdx.x; i0 < total; i0 += blockDim.x * STAGE_BATCH) {
+        uint4 raw[STAGE_BATCH];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            dst[2 * j]     = __uint_as_float(w[j] << 16);
-            dst[2 * j + 1] = __uint_as_float(w[j] & 0xFFFF0000u);
+        for (int t = 0; t < STAGE_BATCH; ++t) {
+            const int i = i0 + t * blockDim.x;
+            const int m = (M == 1) ? 0 : i / nvec, v = (M == 1) ? i : i - m * nvec;
+            raw[t] = make_uint4(0, 0, 0, 0);
+            if (i < total && k_base + v * 8 < p.K)
+                raw[t] = __ldg(reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + k_base + v * 8));
+        }
+#pragma unroll
+        for (int t = 0; t < STAGE_BATCH; ++t) {
+            const int i = i0 + t * blockDim.x;
+            if (i < total) {
+                const int m = (M == 1) ? 0 : i / nvec, v = (M == 1) ? i : i - m * nvec;
+                float* dst = reinterpret_cast<float*>(xs + (size_t)((v >> 2) * M + m) * XBP_W4A16) + (v & 3) * 8;
+                const uint32_t w[4] = {raw[t].x, raw[t].y, raw[t].z, raw[t].w};
+                float4 lo, hi;
+                lo.x = __uint_as_float(w[0] << 16); lo.y = __uint_as_float(w[0] & 0xFFFF0000u);
+                lo.z = __uint_as_float(w[1] << 16); lo.w = __uint_as_float(w[1] & 0xFFFF0000u);
+                hi.x = __uint_as_float(w[2] << 16); hi.y = __uint_as_float(w[2] & 0xFFFF0000u);
+                hi.z = __uint_as_float(w[3] << 16); hi.w = __uint_as_float(w[3] & 0xFFFF0000u);
+                reinterpret_cast<float4*>(dst)[0] = lo;
+                reinterpret_cast<float4*>(dst)[1] = hi;
+            }
         }
     }
 }
 
 // ---- one 32-k vector (two 16-blocks) of R rows against all M activation rows ------------------
 template <int M, int R>
-__device__ __forceinline__ void block_pair_w4a4(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
-                                                int j, float (&acc)[R][M]) {
+__device__ __forceinline__ void block_pair_w4a4(const WLut& lut, const uint4 (&wv)[R], const uint8_t* xbp,
+                                                const float (&sw)[R][8], int j, float (&acc)[R][M]) {
     uint32_t u[R][8];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        decode_w_u8(wv[r].x, u[r][0], u[r][1]);
-        decode_w_u8(wv[r].y, u[r][2], u[r][3]);
-        decode_w_u8(wv[r].z, u[r][4], u[r][5]);
-        decode_w_u8(wv[r].w, u[r][6], u[r][7]);
+        decode_w_u8(lut, wv[r].x, u[r][0], u[r][1]);
+        decode_w_u8(lut, wv[r].y, u[r][2], u[r][3]);
+        decode_w_u8(lut, wv[r].z, u[r][4], u[r][5]);
+        decode_w_u8(lut, wv[r].w, u[r][6], u[r][7]);
     }
 #pragma unroll
     for (int m = 0; m < M; ++m) {
@@ -190,6 +238,70 @@ __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uin
     }
 }
 
+// write one finished unit (R tiles) -- a6 (K parts of a row summed by shuffles) and a7
+template <int M, int R>
+__device__ __forceinline__ void finish_unit(const GemvParams& p, float (&acc)[R][M], int unit, int nvalid, int lane,
+                                            int part, int rsub, int rpt, float gs) {
+    for (int off = 1; off < p.kp; off <<= 1) {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int m = 0; m < M; ++m) acc[r][m] += __shfl_xor_sync(0xFFFFFFFFu, acc[r][m], off);
+    }
+    const bool writer = (part == 0);
+    if (p.ksplit > 1) {
+        // split K: publish the partial; the last warp to arrive for this unit sums all in fixed order
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int n = (unit * R + r) * rpt + rsub;
+            if (writer && r < nvalid) {
+#pragma unroll
+                for (int m = 0; m < M; ++m)
+                    __stcg(p.partials + ((int64_t)blockIdx.y * M + m) * p.Npad + n, acc[r][m]);
+            }
+        }
+        __threadfence();
+        __syncwarp();
+        unsigned int last = 0;
+        if (lane == 0) {
+            const unsigned int old = atomicAdd(p.counters + unit, 1u);
+            last = (old == (unsigned int)p.ksplit - 1u);
+            if (last) p.counters[unit] = 0u;                              // leave the workspace clean
+        }
+        last = __shfl_sync(0xFFFFFFFFu, last, 0);
+        if (!last) return;
+        __threadfence();
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int n = (unit * R + r) * rpt + rsub;
+            if (writer && r < nvalid) {
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    float sum = 0.0f;
+                    for (int ks = 0; ks < p.ksplit; ++ks)
+                        sum += __ldcg(p.partials + ((int64_t)ks * M + m) * p.Npad + n);
+                    acc[r][m] = sum;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int n = (unit * R + r) * rpt + rsub;
+        if (writer && r < nvalid && n < p.N) {
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const float v = acc[r][m] * gs;
+                if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
+                else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
+            }
+        }
+    }
+}
+
+// Persistent, statically balanced: gridDim.x CTAs (about one per SM) share the `units` (R tiles
+// each) evenly; warp w of a CTA walks units u0+w, u0+w+W, ... as ONE flat stream of cells, so its
+// bulk-copy ring never drains between units.
 template <int MODE, int M, int R>
 __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -211,28 +323,44 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
     uint8_t* ring = smem + xs_bytes + (size_t)warp * S * STAGE_BYTES;        // this warp's stages
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + xs_bytes + (size_t)W * S * STAGE_BYTES) + warp * S;
 
-    const int tile0 = (blockIdx.x * W + warp) * R;
-    int nvalid = p.ntiles - tile0;                                           // valid tiles of this warp
-    nvalid = nvalid < 0 ? 0 : (nvalid > R ? R : nvalid);
-    const uint8_t* wsrc = p.blob + ((int64_t)tile0 * p.nch + c0) * CELL_BYTES;
+    // units of this CTA and of this warp
+    const int u0 = (int)(((int64_t)blockIdx.x * p.units) / gridDim.x);
+    const int u1 = (int)(((int64_t)(blockIdx.x + 1) * p.units) / gridDim.x);
+    const int nu = (warp < u1 - u0) ? (u1 - u0 - warp + W - 1) / W : 0;
+    const int total = nu * ncw;                                              // cells this warp consumes
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
 
+    // producer cursor (lane 0 only): next cell to request
+    int p_unit = u0 + warp, p_cell = 0, p_count = 0, p_stage = 0;
+    auto issue = [&]() {
+        const uint32_t bar = smem_u32(bars + p_stage);
+        const int tile0 = p_unit * R;
+        int nv = p.ntiles - tile0; nv = nv > R ? R : nv;
+        mbar_arrive_expect_tx(bar, (uint32_t)nv * CELL_BYTES);
+        const uint8_t* src = p.blob + ((int64_t)tile0 * p.nch + c0 + p_cell) * CELL_BYTES;
+        for (int r = 0; r < nv; ++r)
+            bulk_g2s(smem_u32(ring + (size_t)p_stage * STAGE_BYTES + r * CELL_BYTES), src + r * tile_stride,
+                     CELL_BYTES, bar);
+        ++p_count;
+        if (++p_cell == ncw) { p_cell = 0; p_unit += W; }
+        if (++p_stage == S) p_stage = 0;
+    };
+
     // ---- prologue: start the weight stream before touching the activations ----
-    if (lane == 0 && nvalid > 0) {
+    if (lane == 0 && total > 0) {
         for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
         mbar_fence_init();
-        const int npre = ncw < S ? ncw : S;
-        for (int i = 0; i < npre; ++i) {
-            const uint32_t bar = smem_u32(bars + i);
-            mbar_arrive_expect_tx(bar, (uint32_t)nvalid * CELL_BYTES);
-            for (int r = 0; r < nvalid; ++r)
-                bulk_g2s(smem_u32(ring + (size_t)i * STAGE_BYTES + r * CELL_BYTES),
-                         wsrc + r * tile_stride + (int64_t)i * CELL_BYTES, CELL_BYTES, bar);
-        }
+        const int npre = total < S ? total : S;
+        for (int i = 0; i < npre; ++i) issue();
     }
-    if (MODE == NVFP4_MODE_W4A4) stage_x_w4a4<M>(p, xs, c0, ncw);
-    else                         stage_x_w4a16<M>(p, xs, c0, ncw);
+    if (!(p.dbg & 2)) {
+        if (MODE == NVFP4_MODE_W4A4) stage_x_w4a4<M>(p, xs, c0, ncw);
+        else                         stage_x_w4a16<M>(p, xs, c0, ncw);
+    }
+    float gs = __ldg(p.w_gscale);
+    if (MODE == NVFP4_MODE_W4A4) gs = (gs * __ldg(p.x_gscale)) * 0.25f;     // ints are 2*e on both sides
     __syncthreads();
+    if (total == 0) return;
 
     float acc[R][M];
 #pragma unroll
@@ -240,116 +368,55 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
 #pragma unroll
         for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
 
-    if (nvalid > 0) {
-        int s = 0;
-        uint32_t phase = 0;
-        // this lane's activation records: vector (i*4 + j)*kp + part  ->  stride between j steps = kp records
-        const uint8_t* xlane = xs + (size_t)part * M * XBP;
-        const size_t xstep = (size_t)p.kp * M * XBP;
-        for (int i = 0; i < ncw; ++i) {
-            const uint32_t bar = smem_u32(bars + s);
-            mbar_wait(bar, phase);
-            const uint8_t* st = ring + (size_t)s * STAGE_BYTES;
+    const WLut lut = make_wlut((uint32_t)p.zero);
+    // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
+    const uint8_t* xlane0 = xs + (size_t)part * M * XBP;
+    const size_t xstep = (size_t)p.kp * M * XBP;
+    const uint8_t* xlane = xlane0;
+    int s = 0, c_cell = 0, c_unit = u0 + warp;
+    uint32_t phase = 0;
+    for (int f = 0; f < total; ++f) {
+        const uint32_t bar = smem_u32(bars + s);
+        mbar_wait(bar, phase);
+        const uint8_t* st = ring + (size_t)s * STAGE_BYTES;
 
-            float sw[R][8];
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * 8);
-                const float2 f0 = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
-                const float2 f1 = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
-                const float2 f2 = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
-                const float2 f3 = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
-                sw[r][0] = f0.x; sw[r][1] = f0.y; sw[r][2] = f1.x; sw[r][3] = f1.y;
-                sw[r][4] = f2.x; sw[r][5] = f2.y; sw[r][6] = f3.x; sw[r][7] = f3.y;
-            }
-
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {                                  // four 32-k vectors of this lane
-                uint4 wv[R];
-#pragma unroll
-                for (int r = 0; r < R; ++r)
-                    wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + j * 512 + lane * 16);
-                const uint8_t* xbp = xlane + (size_t)j * xstep;
-                if (MODE == NVFP4_MODE_W4A4) block_pair_w4a4<M, R>(wv, xbp, sw, j, acc);
-                else                         block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
-            }
-            xlane += 4 * xstep;
-
-            // every lane has read stage s -> refill it with cell i+S
-            __syncwarp();
-            if (lane == 0 && i + S < ncw) {
-                mbar_arrive_expect_tx(bar, (uint32_t)nvalid * CELL_BYTES);
-                for (int r = 0; r < nvalid; ++r)
-                    bulk_g2s(smem_u32(ring + (size_t)s * STAGE_BYTES + r * CELL_BYTES),
-                             wsrc + r * tile_stride + (int64_t)(i + S) * CELL_BYTES, CELL_BYTES, bar);
-            }
-            if (++s == S) { s = 0; phase ^= 1u; }
-        }
-    }
-
-    // ---- a6: sum the kp lanes of each row (once) ----
-    for (int off = 1; off < p.kp; off <<= 1) {
-#pragma unroll
-        for (int r = 0; r < R; ++r)
-#pragma unroll
-            for (int m = 0; m < M; ++m) acc[r][m] += __shfl_xor_sync(0xFFFFFFFFu, acc[r][m], off);
-    }
-    const bool writer = (part == 0);
-
-    // ---- a7: epilogue ----
-    float gs = __ldg(p.w_gscale);
-    if (MODE == NVFP4_MODE_W4A4) gs = (gs * __ldg(p.x_gscale)) * 0.25f;     // ints are 2*e on both sides
-
-    if (p.ksplit == 1) {
+        float sw[R][8];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int n = (tile0 + r) * rpt + rsub;
-            if (writer && r < nvalid && n < p.N) {
-#pragma unroll
-                for (int m = 0; m < M; ++m) {
-                    const float v = acc[r][m] * gs;
-                    if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
-                    else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
-                }
-            }
+            const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * 8);
+            const float2 f0 = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
+            const float2 f1 = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
+            const float2 f2 = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
+            const float2 f3 = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
+            sw[r][0] = f0.x; sw[r][1] = f0.y; sw[r][2] = f1.x; sw[r][3] = f1.y;
+            sw[r][4] = f2.x; sw[r][5] = f2.y; sw[r][6] = f3.x; sw[r][7] = f3.y;
         }
-        return;
-    }
+        if (!(p.dbg & 1))
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {                                      // four 32-k vectors of this lane
+            uint4 wv[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + j * 512 + lane * 16);
+            const uint8_t* xbp = xlane + (size_t)j * xstep;
+            if (MODE == NVFP4_MODE_W4A4) block_pair_w4a4<M, R>(lut, wv, xbp, sw, j, acc);
+            else                         block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
+        }
+        xlane += 4 * xstep;
 
-    // split K: publish the partial, the last CTA of this CTA row sums all of them in fixed order
+        // every lane has read stage s -> lane 0 requests the next cell of the flat stream into it
+        __syncwarp();
+        if (lane == 0 && p_count < total) issue();
+        if (++s == S) { s = 0; phase ^= 1u; }
+
+        if (++c_cell == ncw) {                                             // unit finished
+            int nv = p.ntiles - c_unit * R; nv = nv > R ? R : nv;
+            finish_unit<M, R>(p, acc, c_unit, nv, lane, part, rsub, rpt, gs);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int n = (tile0 + r) * rpt + rsub;
-        if (writer && r < nvalid) {
+            for (int r = 0; r < R; ++r)
 #pragma unroll
-            for (int m = 0; m < M; ++m)
-                __stcg(p.partials + ((int64_t)blockIdx.y * M + m) * p.Npad + n, acc[r][m]);
-        }
-    }
-    __shared__ unsigned int s_last;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned int old = atomicAdd(p.counters + blockIdx.x, 1u);
-        s_last = (old == (unsigned int)p.ksplit - 1u);
-        if (s_last) p.counters[blockIdx.x] = 0u;                          // leave the workspace clean
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int n = (tile0 + r) * rpt + rsub;
-        if (writer && r < nvalid && n < p.N) {
-#pragma unroll
-            for (int m = 0; m < M; ++m) {
-                float sum = 0.0f;
-                for (int ks = 0; ks < p.ksplit; ++ks)
-                    sum += __ldcg(p.partials + ((int64_t)ks * M + m) * p.Npad + n);
-                const float v = sum * gs;
-                if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
-                else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
-            }
+                for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
+            c_cell = 0; c_unit += W; xlane = xlane0;
         }
     }
 }
