@@ -9,12 +9,34 @@ constexpr size_t SMEM_CAP = 227 * 1024;
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// arithmetic variant: W4A4 runs the FP16 path up to M = NVFP4_MH (default 1), the integer path above
+int gemv_kmode(int mode, int M) {
+    if (mode == NVFP4_MODE_W4A16) return KMODE_W4A16;
+    static int mh = -1;
+    if (mh < 0) { const char* e = getenv("NVFP4_MH"); mh = e ? atoi(e) : 1; }
+    return M <= mh ? KMODE_W4A4_H : KMODE_W4A4_I8;
+}
+
+// CTAs per K range: about one per SM over all K ranges, never more than there are units
+static int gemv_ctas(int units, const GemvConfig& c) {
+    int ctas = NUM_SMS / c.ksplit;
+    if (ctas < 1) ctas = 1;
+    return ctas > units ? units : ctas;
+}
+
 size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
     const Layout L = make_layout(N, K, layout_kparts(N, K));
     const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
-    const int xbp = (mode == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16;
+    const int xbp = xbp_bytes(gemv_kmode(mode, M));
     const size_t xs = align_up((size_t)ncw_max * 4 * L.kp * M * xbp, 128);
-    return xs + (size_t)c.warps * c.stages * c.rows * CELL_BYTES + (size_t)c.warps * c.stages * 8;
+    const int units = (L.ntiles + c.rows - 1) / c.rows;
+    const int ctas = gemv_ctas(units, c);
+    const int ucta_max = (units + ctas - 1) / ctas;
+    return xs + (size_t)c.warps * c.stages * c.rows * CELL_BYTES             // rings
+         + (size_t)c.warps * 2 * c.rows * M * L.rpt * sizeof(float)          // segment slots
+         + (size_t)c.warps * c.stages * 8                                    // ring mbarriers
+         + ((size_t)ncw_max * L.kp * M * 16 / STAGE_ITEMS + 2) * 8          // staging-batch mbarriers
+         + (size_t)(ucta_max + c.warps + 4) * sizeof(int);                   // unit counters + share starts
 }
 
 // Launch shape per (mode, M, N, K).  Values come from the sweeps recorded in DESIGN.md
@@ -26,15 +48,11 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     if (mode == NVFP4_MODE_W4A4 && M >= 5 && L.ntiles >= 2 * 8 * NUM_SMS) c.rows = 2;
     c.stages = 4;
     c.ksplit = 1;
-    {   // one warp per unit when the units fit one wave of <= 16 warps per SM
-        const int units = (L.ntiles + c.rows - 1) / c.rows;
-        int w = (units + NUM_SMS - 1) / NUM_SMS;
-        c.warps = w < 4 ? 4 : (w > 16 ? 16 : w);
-    }
+    c.warps = 16;
     // shrink until the CTA fits in shared memory: K ranges first when the activations dominate
     while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP / 2) {
         const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
-        const size_t xs = (size_t)ncw_max * 4 * L.kp * M * ((mode == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16);
+        const size_t xs = (size_t)ncw_max * 4 * L.kp * M * xbp_bytes(gemv_kmode(mode, M));
         if (xs > SMEM_CAP / 4 && c.ksplit < L.ncells) ++c.ksplit;
         else if (c.stages > 2) --c.stages;
         else if (gemv_smem_bytes(mode, M, N, K, c) <= SMEM_CAP) break;
@@ -57,6 +75,7 @@ size_t gemv_workspace_bytes_for(int M, int N, int K, const GemvConfig& c) {
 
 cudaError_t launch_gemv_w4a4(const GemvParams& p, int M, int R, dim3 grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t launch_gemv_w4a16(const GemvParams& p, int M, int R, dim3 grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t launch_gemv_w4a4h(const GemvParams& p, int M, int R, dim3 grid, int threads, size_t smem, cudaStream_t st);
 
 cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, const void* x,
                         const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
@@ -77,18 +96,19 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     p.warps = cfg.warps; p.stages = cfg.stages; p.ksplit = cfg.ksplit;
     p.y_bf16 = (y_dtype == NVFP4_DTYPE_BF16);
     p.zero = 0;
-    { const char* e = getenv("NVFP4_DBG"); p.dbg = e ? atoi(e) : 0; }
     if (cfg.ksplit > 1 && ws_bytes < gemv_workspace_bytes_for(M, N, K, cfg)) return cudaErrorInvalidValue;
     const size_t smem = gemv_smem_bytes(mode, M, N, K, cfg);
     if (smem > SMEM_CAP) return cudaErrorInvalidConfiguration;
     p.units = (p.ntiles + cfg.rows - 1) / cfg.rows;
-    int ctas = NUM_SMS / cfg.ksplit;                      // about one CTA per SM over all K ranges
-    { const char* e = getenv("NVFP4_CTAS"); if (e) ctas = atoi(e); }
-    if (ctas < 1) ctas = 1;
-    if (ctas > p.units) ctas = p.units;
+    const int ctas = gemv_ctas(p.units, cfg);
+    // every consumer warp needs at least one cell of the smallest CTA's flat stream
+    const int min_cells = (p.units / ctas) * (p.nch / cfg.ksplit);
+    if (p.warps > min_cells) p.warps = min_cells;
     dim3 grid(ctas, cfg.ksplit);
-    const int threads = cfg.warps * 32;
-    if (mode == NVFP4_MODE_W4A4) return launch_gemv_w4a4(p, M, cfg.rows, grid, threads, smem, st);
+    const int threads = p.warps * 32 + STAGER_THREADS;
+    const int kmode = gemv_kmode(mode, M);
+    if (kmode == KMODE_W4A4_I8) return launch_gemv_w4a4(p, M, cfg.rows, grid, threads, smem, st);
+    if (kmode == KMODE_W4A4_H) return launch_gemv_w4a4h(p, M, cfg.rows, grid, threads, smem, st);
     return launch_gemv_w4a16(p, M, cfg.rows, grid, threads, smem, st);
 }
 

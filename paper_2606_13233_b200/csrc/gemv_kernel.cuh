@@ -42,12 +42,20 @@ struct GemvParams {
     int units;                     // ceil(ntiles / R): work items shared by the gridDim.x CTAs of a K range
     int y_bf16;
     int zero;                      // always 0 (see make_wlut)
-    int dbg;
 };
 
 // shared-memory bytes of activations per 32-k block pair and per m
 constexpr int XBP_W4A4  = 48;    // 32 int8 + {init0, init1, sX0, sX1}
 constexpr int XBP_W4A16 = 128;   // 32 floats
+constexpr int XBP_W4A4H = 80;    // 32 f16 (e2m1 values, exact) + {sX0, sX1} + pad
+
+// kernel arithmetic variants (template parameter MODE of gemv_kernel)
+constexpr int KMODE_W4A4_I8 = 0;   // integer: PRMT LUT decode + dp4a          (best for M >= 2)
+constexpr int KMODE_W4A16   = 1;   // FP32 FMA against BF16 activations
+constexpr int KMODE_W4A4_H  = 2;   // cvt.rn.f16x2.e2m1x2 + HFMA2, exact per 8 k (best for M = 1)
+__host__ __device__ constexpr int xbp_bytes(int kmode) {
+    return kmode == KMODE_W4A4_I8 ? XBP_W4A4 : (kmode == KMODE_W4A16 ? XBP_W4A16 : XBP_W4A4H);
+}
 
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     uint32_t d;
@@ -82,9 +90,20 @@ __device__ __forceinline__ void decode_w_u8(const WLut& l, uint32_t w, uint32_t&
 }
 
 // ---- activation staging: decode the CTA's K range once into shared memory ----------------
-// Loads are issued in batches of STAGE_BATCH per thread before any of them is used, so the L2
-// latency is paid once per batch, not once per block.
+// Done by the CTA's dedicated STAGER warps (threads [W*32, W*32 + STAGER_THREADS)) while the
+// consumer warps already stream and multiply; readiness is signalled per batch through mbarriers.  Loads are issued STAGE_BATCH at a time per thread, so the L2
+// latency is paid once per batch.
 constexpr int STAGE_BATCH = 8;
+constexpr int STAGER_WARPS = 4;
+constexpr int STAGER_THREADS = STAGER_WARPS * 32;
+
+// one mbarrier per staging batch (STAGER_THREADS * STAGE_BATCH work items): every stager thread
+// arrives on it after its stores (release), a consumer waits (acquire) on the batch that contains
+// the last item it needs -- no polling loop, no barrier among the stagers.
+constexpr int STAGE_ITEMS = STAGER_THREADS * STAGE_BATCH;
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 
 __device__ __forceinline__ void decode_x_block(uint2 cw, float sx, uint8_t* base, int half) {
     // nibble -> signed int8 x = 2*e2m1: magnitude LUT through PRMT once per sign, per-byte subtract
@@ -107,20 +126,37 @@ __device__ __forceinline__ void decode_x_block(uint2 cw, float sx, uint8_t* base
     *reinterpret_cast<float*>(base + 40 + half * 4) = sx;
 }
 
-template <int M>
-__device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
+// tid = index among the stager threads.  Work item i -> (block = i / M, m = i % M): progress is
+// monotone in the block index, which is what consumers wait on.
+// FP16 variant of the record: 16 e2m1 values as f16 (8 x F2FP), the block scale as FP32
+__device__ __forceinline__ void decode_x_block_h(uint2 cw, float sx, uint8_t* base, int half) {
+    uint32_t h[8];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        h[b]     = e2m1x2_to_f16x2((cw.x >> (8 * b)) & 0xFFu);
+        h[4 + b] = e2m1x2_to_f16x2((cw.y >> (8 * b)) & 0xFFu);
+    }
+    uint4* dst = reinterpret_cast<uint4*>(base + half * 32);
+    dst[0] = make_uint4(h[0], h[1], h[2], h[3]);
+    dst[1] = make_uint4(h[4], h[5], h[6], h[7]);
+    *reinterpret_cast<float*>(base + 64 + half * 4) = sx;
+}
+
+template <int M, bool HALF>
+__device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
+                                             uint64_t* xbars) {
     const int nblk = ncw * 8 * p.kp;                             // 16-blocks in the range
     const int kb_total = p.K >> 4;
     const int kb0 = c0 * 8 * p.kp;
     const uint8_t* xc = static_cast<const uint8_t*>(p.x);
     const int total = nblk * M;
-    for (int i0 = threadIdx.x; i0 < total; i0 += blockDim.x * STAGE_BATCH) {
+    for (int base = 0; base < total; base += STAGER_THREADS * STAGE_BATCH) {
         uint2 cw[STAGE_BATCH];
         uint32_t sb[STAGE_BATCH];
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = i0 + t * blockDim.x;
-            const int m = (M == 1) ? 0 : i / nblk, blk = (M == 1) ? i : i - m * nblk;
+            const int i = base + t * STAGER_THREADS + tid;
+            const int blk = i / M, m = i - blk * M;
             cw[t] = make_uint2(0u, 0u);
             sb[t] = 0;
             if (i < total && kb0 + blk < kb_total) {
@@ -130,36 +166,40 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
         }
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = i0 + t * blockDim.x;
+            const int i = base + t * STAGER_THREADS + tid;
             if (i < total) {
-                const int m = (M == 1) ? 0 : i / nblk, blk = (M == 1) ? i : i - m * nblk;
-                decode_x_block(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)((blk >> 1) * M + m) * XBP_W4A4, blk & 1);
+                const int blk = i / M, m = i - blk * M;
+                if (HALF) decode_x_block_h(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)((blk >> 1) * M + m) * XBP_W4A4H, blk & 1);
+                else      decode_x_block(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)((blk >> 1) * M + m) * XBP_W4A4, blk & 1);
             }
         }
+        mbar_arrive(smem_u32(xbars + base / STAGE_ITEMS));
     }
 }
 
+// W4A16: work item i -> (8-element vector = i / M, m = i % M); progress published in 16-blocks
 template <int M>
-__device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw) {
+__device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
+                                              uint64_t* xbars) {
     const int nvec = ncw * 16 * p.kp;                            // 8-element vectors per row in the range
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
     const int total = nvec * M;
     const int k_base = c0 * 128 * p.kp;
-    for (int i0 = threadIdx.x; i0 < total; i0 += blockDim.x * STAGE_BATCH) {
+    for (int base = 0; base < total; base += STAGER_THREADS * STAGE_BATCH) {
         uint4 raw[STAGE_BATCH];
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = i0 + t * blockDim.x;
-            const int m = (M == 1) ? 0 : i / nvec, v = (M == 1) ? i : i - m * nvec;
+            const int i = base + t * STAGER_THREADS + tid;
+            const int v = i / M, m = i - v * M;
             raw[t] = make_uint4(0, 0, 0, 0);
             if (i < total && k_base + v * 8 < p.K)
                 raw[t] = __ldg(reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + k_base + v * 8));
         }
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = i0 + t * blockDim.x;
+            const int i = base + t * STAGER_THREADS + tid;
             if (i < total) {
-                const int m = (M == 1) ? 0 : i / nvec, v = (M == 1) ? i : i - m * nvec;
+                const int v = i / M, m = i - v * M;
                 float* dst = reinterpret_cast<float*>(xs + (size_t)((v >> 2) * M + m) * XBP_W4A16) + (v & 3) * 8;
                 const uint32_t w[4] = {raw[t].x, raw[t].y, raw[t].z, raw[t].w};
                 float4 lo, hi;
@@ -171,6 +211,7 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
                 reinterpret_cast<float4*>(dst)[1] = hi;
             }
         }
+        mbar_arrive(smem_u32(xbars + base / STAGE_ITEMS));
     }
 }
 
@@ -201,6 +242,60 @@ __device__ __forceinline__ void block_pair_w4a4(const WLut& lut, const uint4 (&w
             d1 = dp4a_us(u[r][6], xb.z, d1); d1 = dp4a_us(u[r][7], xb.w, d1);
             acc[r][m] = fmaf((float)d0, sw[r][2 * j] * sx0, acc[r][m]);
             acc[r][m] = fmaf((float)d1, sw[r][2 * j + 1] * sx1, acc[r][m]);
+        }
+    }
+}
+
+// FP16 variant: F2FP.E2M1 unpack (free byte select) + HFMA2.  A half2 lane sums 8 products per
+// 16-block: multiples of 0.25 bounded by 288, exact in FP16; the two lanes are added in FP32.
+__device__ __forceinline__ uint32_t hfma2(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ void cvt_word_e2m1(uint32_t w, uint32_t (&h)[4]) {
+    asm("{.reg .b8 t0,t1,t2,t3; mov.b32 {t0,t1,t2,t3}, %4;\n"
+        "cvt.rn.f16x2.e2m1x2 %0, t0; cvt.rn.f16x2.e2m1x2 %1, t1; cvt.rn.f16x2.e2m1x2 %2, t2; cvt.rn.f16x2.e2m1x2 %3, t3;}"
+        : "=r"(h[0]), "=r"(h[1]), "=r"(h[2]), "=r"(h[3]) : "r"(w));
+}
+__device__ __forceinline__ float2 h2_to_float2(uint32_t h2) {
+    float2 r;
+    asm("{.reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi;}"
+        : "=f"(r.x), "=f"(r.y) : "r"(h2));
+    return r;
+}
+template <int M, int R>
+__device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
+                                                  int j, float (&acc)[R][M]) {
+    uint32_t wh[R][16];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        uint32_t t[4];
+        cvt_word_e2m1(wv[r].x, t); wh[r][0] = t[0]; wh[r][1] = t[1]; wh[r][2] = t[2]; wh[r][3] = t[3];
+        cvt_word_e2m1(wv[r].y, t); wh[r][4] = t[0]; wh[r][5] = t[1]; wh[r][6] = t[2]; wh[r][7] = t[3];
+        cvt_word_e2m1(wv[r].z, t); wh[r][8] = t[0]; wh[r][9] = t[1]; wh[r][10] = t[2]; wh[r][11] = t[3];
+        cvt_word_e2m1(wv[r].w, t); wh[r][12] = t[0]; wh[r][13] = t[1]; wh[r][14] = t[2]; wh[r][15] = t[3];
+    }
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const uint4* xr = reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4H);
+        const uint4 x0 = xr[0], x1 = xr[1], x2 = xr[2], x3 = xr[3];
+        const float2 sx = *reinterpret_cast<const float2*>(xbp + m * XBP_W4A4H + 64);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            uint32_t a0 = 0u, a1 = 0u;
+            a0 = hfma2(wh[r][0], x0.x, a0); a0 = hfma2(wh[r][1], x0.y, a0);
+            a0 = hfma2(wh[r][2], x0.z, a0); a0 = hfma2(wh[r][3], x0.w, a0);
+            a0 = hfma2(wh[r][4], x1.x, a0); a0 = hfma2(wh[r][5], x1.y, a0);
+            a0 = hfma2(wh[r][6], x1.z, a0); a0 = hfma2(wh[r][7], x1.w, a0);
+            a1 = hfma2(wh[r][8], x2.x, a1); a1 = hfma2(wh[r][9], x2.y, a1);
+            a1 = hfma2(wh[r][10], x2.z, a1); a1 = hfma2(wh[r][11], x2.w, a1);
+            a1 = hfma2(wh[r][12], x3.x, a1); a1 = hfma2(wh[r][13], x3.y, a1);
+            a1 = hfma2(wh[r][14], x3.z, a1); a1 = hfma2(wh[r][15], x3.w, a1);
+            const float2 f0 = h2_to_float2(a0), f1 = h2_to_float2(a1);
+            const float p0 = sw[r][2 * j] * sx.x, p1 = sw[r][2 * j + 1] * sx.y;
+            acc[r][m] = fmaf(f0.x, p0, acc[r][m]); acc[r][m] = fmaf(f0.y, p0, acc[r][m]);
+            acc[r][m] = fmaf(f1.x, p1, acc[r][m]); acc[r][m] = fmaf(f1.y, p1, acc[r][m]);
         }
     }
 }
@@ -238,19 +333,15 @@ __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uin
     }
 }
 
-// write one finished unit (R tiles) -- a6 (K parts of a row summed by shuffles) and a7
+// ---- a7: write one finished unit (R tiles); `acc` holds the unit's complete sums over this CTA's
+// K range in the writer lanes (part == 0).  With split K across CTAs (grid.y > 1) the FP32 partial
+// goes to the workspace and the last warp to arrive for this unit sums all K ranges in fixed order.
 template <int M, int R>
-__device__ __forceinline__ void finish_unit(const GemvParams& p, float (&acc)[R][M], int unit, int nvalid, int lane,
-                                            int part, int rsub, int rpt, float gs) {
-    for (int off = 1; off < p.kp; off <<= 1) {
-#pragma unroll
-        for (int r = 0; r < R; ++r)
-#pragma unroll
-            for (int m = 0; m < M; ++m) acc[r][m] += __shfl_xor_sync(0xFFFFFFFFu, acc[r][m], off);
-    }
-    const bool writer = (part == 0);
+__device__ __forceinline__ void emit_unit(const GemvParams& p, float (&acc)[R][M], int unit, int lane, bool writer,
+                                          int rsub, int rpt, float gs) {
+    int nvalid = p.ntiles - unit * R;
+    nvalid = nvalid > R ? R : nvalid;
     if (p.ksplit > 1) {
-        // split K: publish the partial; the last warp to arrive for this unit sums all in fixed order
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int n = (unit * R + r) * rpt + rsub;
@@ -299,17 +390,80 @@ __device__ __forceinline__ void finish_unit(const GemvParams& p, float (&acc)[R]
     }
 }
 
-// Persistent, statically balanced: gridDim.x CTAs (about one per SM) share the `units` (R tiles
-// each) evenly; warp w of a CTA walks units u0+w, u0+w+W, ... as ONE flat stream of cells, so its
-// bulk-copy ring never drains between units.
+// first cell of consumer warp w's share of the CTA's flat stream of T cells (W <= T <= 2^26)
+__device__ __forceinline__ int flat_start(int w, int T, int W) { return (int)(((unsigned)w * (unsigned)T) / (unsigned)W); }
+
+// ---- a6: a warp finished its segment [cells seg_c0 .. seg_c1] of unit `ul` (CTA-local index).
+// K parts of a row are summed by shuffles; a unit shared by several warps is combined through
+// shared-memory slots (two per warp: slot 0 = the segment that starts the warp's share, slot 1 =
+// any later one) by the LAST warp to arrive, in fixed warp order -> deterministic.
+template <int M, int R>
+__device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)[R][M], float* slots, int* cnt,
+                                               const int* fstart,
+                                               int ul, int unit, bool whole, bool seg_at_share_start, int ncw, int T,
+                                               int warp, int lane, int part, int rsub, int rpt, float gs) {
+    for (int off = 1; off < p.kp; off <<= 1) {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int m = 0; m < M; ++m) acc[r][m] += __shfl_xor_sync(0xFFFFFFFFu, acc[r][m], off);
+    }
+    const bool writer = (part == 0);
+    if (!whole) {
+        const int W = p.warps;
+        const int slot_floats = R * M * rpt;
+        float* mine = slots + (size_t)(warp * 2 + (seg_at_share_start ? 0 : 1)) * slot_floats;
+        if (writer) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int m = 0; m < M; ++m) mine[(r * M + m) * rpt + rsub] = acc[r][m];
+        }
+        // contributors of this unit: warps whose share intersects [ul*ncw, (ul+1)*ncw)
+        const int lo = ul * ncw, hi = lo + ncw - 1;
+        int w_first = 0, w_last = 0;
+        for (int w = 0; w < W; ++w) {
+            const int fs = fstart[w];
+            if (fs <= lo) w_first = w;
+            if (fs <= hi) w_last = w;
+        }
+        __threadfence_block();
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) last = (atomicAdd(cnt + ul, 1) == w_last - w_first);
+        last = __shfl_sync(0xFFFFFFFFu, last, 0);
+        if (!last) return;
+        __threadfence_block();
+        if (writer) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
+            for (int w = w_first; w <= w_last; ++w) {
+                const float* sl = slots + (size_t)(w * 2 + (fstart[w] >= lo ? 0 : 1)) * slot_floats;
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int m = 0; m < M; ++m) acc[r][m] += *(volatile const float*)(sl + (r * M + m) * rpt + rsub);
+            }
+        }
+    }
+    emit_unit<M, R>(p, acc, unit, lane, writer, rsub, rpt, gs);
+}
+
+// Persistent and statically balanced.  gridDim.x CTAs (about one per SM) share the `units` (R tiles
+// each) evenly; inside a CTA the flat stream of T = units_cta * ncw cells is cut into W equal
+// shares, one per consumer warp, so every warp does the same amount of work whatever the shape
+// (a unit cut between warps is recombined in finish_segment).  A warp's bulk-copy ring runs over
+// its whole share and never drains between units.  STAGER_WARPS extra warps decode the activations.
 template <int MODE, int M, int R>
-__global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
+__global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
     const int part = lane & (p.kp - 1), rsub = lane >> p.kp_shift;          // lane = rsub*kp + part
     const int rpt = 32 >> p.kp_shift;
-    constexpr int XBP = (MODE == NVFP4_MODE_W4A4) ? XBP_W4A4 : XBP_W4A16;
+    constexpr int XBP = xbp_bytes(MODE);
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
 
     // K range of this CTA (whole cells of 128*kp k)
@@ -318,23 +472,49 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
     const int ncw = c1 - c0;
     const int ncw_max = (p.nch + p.ksplit - 1) / p.ksplit;
 
-    uint8_t* xs = smem;                                                      // activations
-    const size_t xs_bytes = ((size_t)ncw_max * 4 * p.kp * M * XBP + 127) & ~(size_t)127;
-    uint8_t* ring = smem + xs_bytes + (size_t)warp * S * STAGE_BYTES;        // this warp's stages
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + xs_bytes + (size_t)W * S * STAGE_BYTES) + warp * S;
-
-    // units of this CTA and of this warp
+    // units of this CTA
     const int u0 = (int)(((int64_t)blockIdx.x * p.units) / gridDim.x);
     const int u1 = (int)(((int64_t)(blockIdx.x + 1) * p.units) / gridDim.x);
-    const int nu = (warp < u1 - u0) ? (u1 - u0 - warp + W - 1) / W : 0;
-    const int total = nu * ncw;                                              // cells this warp consumes
+    const int ucta_max = (p.units + gridDim.x - 1) / gridDim.x;
+    const int T = (u1 - u0) * ncw;                                          // cells of this CTA (>= W)
+
+    // shared memory carve-up (must match gemv_smem_bytes)
+    uint8_t* xs = smem;                                                      // activations
+    const size_t xs_bytes = ((size_t)ncw_max * 4 * p.kp * M * XBP + 127) & ~(size_t)127;
+    uint8_t* ring_all = smem + xs_bytes;
+    float* slots = reinterpret_cast<float*>(ring_all + (size_t)W * S * STAGE_BYTES);
+    uint64_t* bars_all = reinterpret_cast<uint64_t*>(slots + (size_t)W * 2 * R * M * rpt);
+    const int xitems = ncw_max * p.kp * M * ((MODE == KMODE_W4A16) ? 16 : 8);  // staging work items (upper bound)
+    const int nxb = (xitems + STAGE_ITEMS - 1) / STAGE_ITEMS;
+    uint64_t* xbars = bars_all + W * S;
+    int* cnt = reinterpret_cast<int*>(xbars + nxb);
+    int* fstart = cnt + ucta_max;
+
+    for (int i = threadIdx.x; i < ucta_max; i += blockDim.x) cnt[i] = 0;
+    if (threadIdx.x <= W) fstart[threadIdx.x] = flat_start(threadIdx.x, T, W);
+    if (threadIdx.x < nxb) mbar_init(smem_u32(xbars + threadIdx.x), STAGER_THREADS);
+    if (threadIdx.x == 0) mbar_fence_init();
+    __syncthreads();
+
+    if (warp >= W) {                                                        // ---- stager warps ----
+        const int tid = threadIdx.x - W * 32;
+        if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, tid, xbars);
+        else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, tid, xbars);
+        return;
+    }
+
+    // ---- consumer warps ----
+    uint8_t* ring = ring_all + (size_t)warp * S * STAGE_BYTES;
+    uint64_t* bars = bars_all + warp * S;
+    const int f0 = fstart[warp], f1 = fstart[warp + 1];
+    const int total = f1 - f0;
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
 
-    // producer cursor (lane 0 only): next cell to request
-    int p_unit = u0 + warp, p_cell = 0, p_count = 0, p_stage = 0;
+    // producer cursor (used by lane 0 only): next cell to request
+    int p_ul = f0 / ncw, p_cell = f0 - p_ul * ncw, p_count = 0, p_stage = 0;
     auto issue = [&]() {
         const uint32_t bar = smem_u32(bars + p_stage);
-        const int tile0 = p_unit * R;
+        const int tile0 = (u0 + p_ul) * R;
         int nv = p.ntiles - tile0; nv = nv > R ? R : nv;
         mbar_arrive_expect_tx(bar, (uint32_t)nv * CELL_BYTES);
         const uint8_t* src = p.blob + ((int64_t)tile0 * p.nch + c0 + p_cell) * CELL_BYTES;
@@ -342,25 +522,18 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
             bulk_g2s(smem_u32(ring + (size_t)p_stage * STAGE_BYTES + r * CELL_BYTES), src + r * tile_stride,
                      CELL_BYTES, bar);
         ++p_count;
-        if (++p_cell == ncw) { p_cell = 0; p_unit += W; }
+        if (++p_cell == ncw) { p_cell = 0; ++p_ul; }
         if (++p_stage == S) p_stage = 0;
     };
-
-    // ---- prologue: start the weight stream before touching the activations ----
-    if (lane == 0 && total > 0) {
+    if (lane == 0) {                                                        // start the weight stream first
         for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
         mbar_fence_init();
         const int npre = total < S ? total : S;
         for (int i = 0; i < npre; ++i) issue();
     }
-    if (!(p.dbg & 2)) {
-        if (MODE == NVFP4_MODE_W4A4) stage_x_w4a4<M>(p, xs, c0, ncw);
-        else                         stage_x_w4a16<M>(p, xs, c0, ncw);
-    }
     float gs = __ldg(p.w_gscale);
-    if (MODE == NVFP4_MODE_W4A4) gs = (gs * __ldg(p.x_gscale)) * 0.25f;     // ints are 2*e on both sides
-    __syncthreads();
-    if (total == 0) return;
+    if (MODE == KMODE_W4A4_I8) gs = (gs * __ldg(p.x_gscale)) * 0.25f;       // ints are 2*e on both sides
+    if (MODE == KMODE_W4A4_H)  gs = gs * __ldg(p.x_gscale);
 
     float acc[R][M];
 #pragma unroll
@@ -370,12 +543,20 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
 
     const WLut lut = make_wlut((uint32_t)p.zero);
     // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
-    const uint8_t* xlane0 = xs + (size_t)part * M * XBP;
     const size_t xstep = (size_t)p.kp * M * XBP;
-    const uint8_t* xlane = xlane0;
-    int s = 0, c_cell = 0, c_unit = u0 + warp;
+    const uint8_t* xlane0 = xs + (size_t)part * M * XBP;
+    int c_ul = f0 / ncw, c_cell = f0 - c_ul * ncw;
+    const uint8_t* xlane = xlane0 + (size_t)c_cell * 4 * xstep;
+    int seg_c0 = c_cell;                                                    // first cell of the current segment
+    bool seg_first = true;                                                  // segment starts at the share start
+    int xb_seen = -1;                                                       // last staging batch known complete
+    constexpr int ITEMS_PER_CELL_KP = M * ((MODE == KMODE_W4A16) ? 16 : 8); // staging items per cell and K part
+    int s = 0;
     uint32_t phase = 0;
+    __syncwarp();
     for (int f = 0; f < total; ++f) {
+        const int xb_need = ((c_cell + 1) * p.kp * ITEMS_PER_CELL_KP - 1) / STAGE_ITEMS;   // batch of the last item
+        while (xb_seen < xb_need) { ++xb_seen; mbar_wait(smem_u32(xbars + xb_seen), 0u); }
         const uint32_t bar = smem_u32(bars + s);
         mbar_wait(bar, phase);
         const uint8_t* st = ring + (size_t)s * STAGE_BYTES;
@@ -384,14 +565,13 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * 8);
-            const float2 f0 = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
-            const float2 f1 = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
-            const float2 f2 = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
-            const float2 f3 = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
-            sw[r][0] = f0.x; sw[r][1] = f0.y; sw[r][2] = f1.x; sw[r][3] = f1.y;
-            sw[r][4] = f2.x; sw[r][5] = f2.y; sw[r][6] = f3.x; sw[r][7] = f3.y;
+            const float2 f0s = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
+            const float2 f1s = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
+            const float2 f2s = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
+            const float2 f3s = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
+            sw[r][0] = f0s.x; sw[r][1] = f0s.y; sw[r][2] = f1s.x; sw[r][3] = f1s.y;
+            sw[r][4] = f2s.x; sw[r][5] = f2s.y; sw[r][6] = f3s.x; sw[r][7] = f3s.y;
         }
-        if (!(p.dbg & 1))
 #pragma unroll
         for (int j = 0; j < 4; ++j) {                                      // four 32-k vectors of this lane
             uint4 wv[R];
@@ -399,25 +579,29 @@ __global__ void __launch_bounds__(512) gemv_kernel(const GemvParams p) {
             for (int r = 0; r < R; ++r)
                 wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + j * 512 + lane * 16);
             const uint8_t* xbp = xlane + (size_t)j * xstep;
-            if (MODE == NVFP4_MODE_W4A4) block_pair_w4a4<M, R>(lut, wv, xbp, sw, j, acc);
-            else                         block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
+            if (MODE == KMODE_W4A4_I8)     block_pair_w4a4<M, R>(lut, wv, xbp, sw, j, acc);
+            else if (MODE == KMODE_W4A4_H) block_pair_w4a4_h<M, R>(wv, xbp, sw, j, acc);
+            else                           block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
         }
         xlane += 4 * xstep;
 
-        // every lane has read stage s -> lane 0 requests the next cell of the flat stream into it
+        // every lane has read stage s -> lane 0 requests the next cell of the share into it
         __syncwarp();
         if (lane == 0 && p_count < total) issue();
         if (++s == S) { s = 0; phase ^= 1u; }
 
-        if (++c_cell == ncw) {                                             // unit finished
-            int nv = p.ntiles - c_unit * R; nv = nv > R ? R : nv;
-            finish_unit<M, R>(p, acc, c_unit, nv, lane, part, rsub, rpt, gs);
+        const bool unit_end = (c_cell + 1 == ncw);
+        if (unit_end || f + 1 == total) {                                   // segment finished
+            finish_segment<M, R>(p, acc, slots, cnt, fstart, c_ul, u0 + c_ul, seg_c0 == 0 && unit_end, seg_first, ncw, T,
+                                 warp, lane, part, rsub, rpt, gs);
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
-            c_cell = 0; c_unit += W; xlane = xlane0;
+            seg_first = false;
+            seg_c0 = 0;
         }
+        if (unit_end) { c_cell = 0; ++c_ul; xlane = xlane0; } else ++c_cell;
     }
 }
 

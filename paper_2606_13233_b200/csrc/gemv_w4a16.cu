@@ -1,10 +1,10 @@
-// gemv_w4a16.cu -- instantiates the W4A16 GEMV kernels (all M = 1..8, R = 1, 2, 4).
+// gemv_w4a16.cu -- instantiates the KMODE_W4A16 GEMV kernels (all M = 1..8, R = 1, 2, 4).
 #include "gemv_dispatch.cuh"
 
 namespace nvfp4 {
 
 cudaError_t launch_gemv_w4a16(const GemvParams& p, int M, int R, dim3 grid, int threads, size_t smem, cudaStream_t st) {
-    return launch_m<NVFP4_MODE_W4A16>(p, M, R, grid, threads, smem, st);
+    return launch_m<KMODE_W4A16>(p, M, R, grid, threads, smem, st);
 }
 
 }  // namespace nvfp4
