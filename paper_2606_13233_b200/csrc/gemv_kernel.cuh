@@ -253,6 +253,16 @@ __device__ __forceinline__ uint32_t hfma2(uint32_t a, uint32_t b, uint32_t c) {
     asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
     return d;
 }
+__device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
+    uint32_t d;
+    asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+    return d;
+}
+__device__ __forceinline__ uint32_t hadd2(uint32_t a, uint32_t b) {
+    uint32_t d;
+    asm("add.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+    return d;
+}
 __device__ __forceinline__ void cvt_word_e2m1(uint32_t w, uint32_t (&h)[4]) {
     asm("{.reg .b8 t0,t1,t2,t3; mov.b32 {t0,t1,t2,t3}, %4;\n"
         "cvt.rn.f16x2.e2m1x2 %0, t0; cvt.rn.f16x2.e2m1x2 %1, t1; cvt.rn.f16x2.e2m1x2 %2, t2; cvt.rn.f16x2.e2m1x2 %3, t3;}"
@@ -283,15 +293,16 @@ __device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const ui
         const float2 sx = *reinterpret_cast<const float2*>(xbp + m * XBP_W4A4H + 64);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            uint32_t a0 = 0u, a1 = 0u;
-            a0 = hfma2(wh[r][0], x0.x, a0); a0 = hfma2(wh[r][1], x0.y, a0);
-            a0 = hfma2(wh[r][2], x0.z, a0); a0 = hfma2(wh[r][3], x0.w, a0);
-            a0 = hfma2(wh[r][4], x1.x, a0); a0 = hfma2(wh[r][5], x1.y, a0);
-            a0 = hfma2(wh[r][6], x1.z, a0); a0 = hfma2(wh[r][7], x1.w, a0);
-            a1 = hfma2(wh[r][8], x2.x, a1); a1 = hfma2(wh[r][9], x2.y, a1);
-            a1 = hfma2(wh[r][10], x2.z, a1); a1 = hfma2(wh[r][11], x2.w, a1);
-            a1 = hfma2(wh[r][12], x3.x, a1); a1 = hfma2(wh[r][13], x3.y, a1);
-            a1 = hfma2(wh[r][14], x3.z, a1); a1 = hfma2(wh[r][15], x3.w, a1);
+            // two independent 4-deep chains per block, merged by an exact HADD2 (|sums| <= 288)
+            uint32_t a0 = hmul2(wh[r][0], x0.x), b0 = hmul2(wh[r][4], x1.x);
+            uint32_t a1 = hmul2(wh[r][8], x2.x), b1 = hmul2(wh[r][12], x3.x);
+            a0 = hfma2(wh[r][1], x0.y, a0); b0 = hfma2(wh[r][5], x1.y, b0);
+            a1 = hfma2(wh[r][9], x2.y, a1); b1 = hfma2(wh[r][13], x3.y, b1);
+            a0 = hfma2(wh[r][2], x0.z, a0); b0 = hfma2(wh[r][6], x1.z, b0);
+            a1 = hfma2(wh[r][10], x2.z, a1); b1 = hfma2(wh[r][14], x3.z, b1);
+            a0 = hfma2(wh[r][3], x0.w, a0); b0 = hfma2(wh[r][7], x1.w, b0);
+            a1 = hfma2(wh[r][11], x2.w, a1); b1 = hfma2(wh[r][15], x3.w, b1);
+            a0 = hadd2(a0, b0); a1 = hadd2(a1, b1);
             const float2 f0 = h2_to_float2(a0), f1 = h2_to_float2(a1);
             const float p0 = sw[r][2 * j] * sx.x, p1 = sw[r][2 * j + 1] * sx.y;
             acc[r][m] = fmaf(f0.x, p0, acc[r][m]); acc[r][m] = fmaf(f0.y, p0, acc[r][m]);
@@ -510,22 +521,37 @@ __global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
     const int total = f1 - f0;
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
 
-    // producer cursor (used by lane 0 only): next cell to request
-    int p_ul = f0 / ncw, p_cell = f0 - p_ul * ncw, p_count = 0, p_stage = 0;
+    // producer cursor (used by lane 0 only): next cell to request.  Within a unit the cells of a
+    // tile are contiguous in the blob; with ksplit == 1 and R == 1 the whole share is one run.
+    const bool leader = (lane == 0);
+    int p_left = 0, p_count = 0, p_nv = 0;
+    uint32_t p_dst = smem_u32(ring), p_bar = smem_u32(bars);
+    const uint32_t ring_end = p_dst + (uint32_t)S * STAGE_BYTES;
+    const uint8_t* p_src = nullptr;
+    {
+        const int ul = f0 / ncw, cell = f0 - ul * ncw;
+        const int tile0 = (u0 + ul) * R;
+        p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
+        p_left = ncw - cell;
+        p_nv = p.ntiles - tile0; p_nv = p_nv > R ? R : p_nv;
+    }
+    const int64_t unit_jump = (int64_t)(R - 1) * tile_stride + (int64_t)(p.nch - ncw) * CELL_BYTES;
     auto issue = [&]() {
-        const uint32_t bar = smem_u32(bars + p_stage);
-        const int tile0 = (u0 + p_ul) * R;
-        int nv = p.ntiles - tile0; nv = nv > R ? R : nv;
-        mbar_arrive_expect_tx(bar, (uint32_t)nv * CELL_BYTES);
-        const uint8_t* src = p.blob + ((int64_t)tile0 * p.nch + c0 + p_cell) * CELL_BYTES;
-        for (int r = 0; r < nv; ++r)
-            bulk_g2s(smem_u32(ring + (size_t)p_stage * STAGE_BYTES + r * CELL_BYTES), src + r * tile_stride,
-                     CELL_BYTES, bar);
+        mbar_arrive_expect_tx(p_bar, (uint32_t)p_nv * CELL_BYTES);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (r < p_nv) bulk_g2s(p_dst + r * CELL_BYTES, p_src + r * tile_stride, CELL_BYTES, p_bar);
         ++p_count;
-        if (++p_cell == ncw) { p_cell = 0; ++p_ul; }
-        if (++p_stage == S) p_stage = 0;
+        p_src += CELL_BYTES;
+        if (--p_left == 0) {                                                // next unit of the share
+            p_src += unit_jump;
+            p_left = ncw;
+            if (R > 1) { p_nv = p.ntiles - (int)((p_src - p.blob) / tile_stride); p_nv = p_nv > R ? R : p_nv; }
+        }
+        p_dst += STAGE_BYTES; p_bar += 8;
+        if (p_dst == ring_end) { p_dst -= (uint32_t)S * STAGE_BYTES; p_bar -= (uint32_t)S * 8; }
     };
-    if (lane == 0) {                                                        // start the weight stream first
+    if (leader) {                                                           // start the weight stream first
         for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
         mbar_fence_init();
         const int npre = total < S ? total : S;
@@ -545,21 +571,26 @@ __global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
     // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
     const size_t xstep = (size_t)p.kp * M * XBP;
     const uint8_t* xlane0 = xs + (size_t)part * M * XBP;
-    int c_ul = f0 / ncw, c_cell = f0 - c_ul * ncw;
-    const uint8_t* xlane = xlane0 + (size_t)c_cell * 4 * xstep;
-    int seg_c0 = c_cell;                                                    // first cell of the current segment
-    bool seg_first = true;                                                  // segment starts at the share start
-    int xb_seen = -1;                                                       // last staging batch known complete
-    constexpr int ITEMS_PER_CELL_KP = M * ((MODE == KMODE_W4A16) ? 16 : 8); // staging items per cell and K part
-    int s = 0;
+    int c_ul = f0 / ncw;
+    const int cell0 = f0 - c_ul * ncw;
+    const uint8_t* xlane = xlane0 + (size_t)cell0 * 4 * xstep;
+    // loop state kept incremental (no per-iteration index arithmetic): consumer stage pointer and
+    // barrier, cells left in the current segment, staging items this lane's next cell depends on
+    const uint8_t* st = ring;
+    const uint8_t* const st_end = ring + (size_t)S * STAGE_BYTES;
+    uint32_t bar = smem_u32(bars);
     uint32_t phase = 0;
+    int seg_left = (ncw - cell0) < total ? (ncw - cell0) : total;           // cells until the segment ends
+    bool seg_first = true, seg_from0 = (cell0 == 0);
+    constexpr int ITEMS_PER_CELL_KP = M * ((MODE == KMODE_W4A16) ? 16 : 8); // staging items per cell and K part
+    const int x_items_cell = p.kp * ITEMS_PER_CELL_KP;
+    int x_need = (cell0 + 1) * x_items_cell;                                // items that must be staged
+    int x_have = 0;                                                         // items known to be staged
+    uint32_t xbar = smem_u32(xbars);
     __syncwarp();
     for (int f = 0; f < total; ++f) {
-        const int xb_need = ((c_cell + 1) * p.kp * ITEMS_PER_CELL_KP - 1) / STAGE_ITEMS;   // batch of the last item
-        while (xb_seen < xb_need) { ++xb_seen; mbar_wait(smem_u32(xbars + xb_seen), 0u); }
-        const uint32_t bar = smem_u32(bars + s);
+        while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += STAGE_ITEMS; }
         mbar_wait(bar, phase);
-        const uint8_t* st = ring + (size_t)s * STAGE_BYTES;
 
         float sw[R][8];
 #pragma unroll
@@ -584,24 +615,27 @@ __global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
             else                           block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
         }
         xlane += 4 * xstep;
+        x_need += x_items_cell;
 
-        // every lane has read stage s -> lane 0 requests the next cell of the share into it
+        // every lane has read the stage -> lane 0 requests the next cell of the share into it
         __syncwarp();
-        if (lane == 0 && p_count < total) issue();
-        if (++s == S) { s = 0; phase ^= 1u; }
+        if (leader && p_count < total) issue();
+        st += STAGE_BYTES; bar += 8;
+        if (st == st_end) { st = ring; bar -= (uint32_t)S * 8; phase ^= 1u; }
 
-        const bool unit_end = (c_cell + 1 == ncw);
-        if (unit_end || f + 1 == total) {                                   // segment finished
-            finish_segment<M, R>(p, acc, slots, cnt, fstart, c_ul, u0 + c_ul, seg_c0 == 0 && unit_end, seg_first, ncw, T,
+        if (--seg_left == 0) {                                              // segment finished
+            const int left = total - f - 1;
+            const bool unit_end = (left == 0) ? (x_need - x_items_cell == ncw * x_items_cell) : true;
+            finish_segment<M, R>(p, acc, slots, cnt, fstart, c_ul, u0 + c_ul, seg_from0 && unit_end, seg_first, ncw, T,
                                  warp, lane, part, rsub, rpt, gs);
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
-            seg_first = false;
-            seg_c0 = 0;
+            seg_first = false; seg_from0 = true;
+            seg_left = left < ncw ? left : ncw;
+            ++c_ul; xlane = xlane0; x_need = x_items_cell;
         }
-        if (unit_end) { c_cell = 0; ++c_ul; xlane = xlane0; } else ++c_cell;
     }
 }
 
