@@ -48,7 +48,7 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     if (mode == NVFP4_MODE_W4A4 && M >= 5 && L.ntiles >= 2 * 8 * NUM_SMS) c.rows = 2;
     c.stages = 4;
     c.ksplit = 1;
-    c.warps = 16;
+    c.warps = (M <= 2) ? 16 : 12;
     // shrink until the CTA fits in shared memory: K ranges first when the activations dominate
     while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP / 2) {
         const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
@@ -104,6 +104,7 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     // every consumer warp needs at least one cell of the smallest CTA's flat stream
     const int min_cells = (p.units / ctas) * (p.nch / cfg.ksplit);
     if (p.warps > min_cells) p.warps = min_cells;
+    if (M > 1 && p.warps > 16) p.warps = 16;             // launch bounds: 1024 threads for M = 1, 640 otherwise
     dim3 grid(ctas, cfg.ksplit);
     const int threads = p.warps * 32 + STAGER_THREADS;
     const int kmode = gemv_kmode(mode, M);

@@ -438,13 +438,15 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
             if (fs <= lo) w_first = w;
             if (fs <= hi) w_last = w;
         }
-        __threadfence_block();
-        __syncwarp();
+        __syncwarp();                                   // the writer lanes' slot stores are ordered before ...
         int last = 0;
-        if (lane == 0) last = (atomicAdd(cnt + ul, 1) == w_last - w_first);
+        if (lane == 0) {                                // ... this CTA-scope acq_rel arrival (no separate fences)
+            int old;
+            asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(cnt + ul)) : "memory");
+            last = (old == w_last - w_first);
+        }
         last = __shfl_sync(0xFFFFFFFFu, last, 0);
         if (!last) return;
-        __threadfence_block();
         if (writer) {
 #pragma unroll
             for (int r = 0; r < R; ++r)
@@ -468,7 +470,7 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
 // (a unit cut between warps is recombined in finish_segment).  A warp's bulk-copy ring runs over
 // its whole share and never drains between units.  STAGER_WARPS extra warps decode the activations.
 template <int MODE, int M, int R>
-__global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
+__global__ void __launch_bounds__(M == 1 ? 1024 : 640) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
@@ -557,9 +559,9 @@ __global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
         const int npre = total < S ? total : S;
         for (int i = 0; i < npre; ++i) issue();
     }
-    float gs = __ldg(p.w_gscale);
-    if (MODE == KMODE_W4A4_I8) gs = (gs * __ldg(p.x_gscale)) * 0.25f;       // ints are 2*e on both sides
-    if (MODE == KMODE_W4A4_H)  gs = gs * __ldg(p.x_gscale);
+    // global scales: issue the loads now, combine them only when the first segment is written
+    const float gw_raw = __ldg(p.w_gscale);
+    const float gx_raw = (MODE == KMODE_W4A16) ? 1.0f : __ldg(p.x_gscale);
 
     float acc[R][M];
 #pragma unroll
@@ -624,6 +626,9 @@ __global__ void __launch_bounds__(640) gemv_kernel(const GemvParams p) {
         if (st == st_end) { st = ring; bar -= (uint32_t)S * 8; phase ^= 1u; }
 
         if (--seg_left == 0) {                                              // segment finished
+            float gs = gw_raw;
+            if (MODE == KMODE_W4A4_I8) gs = (gs * gx_raw) * 0.25f;          // ints are 2*e on both sides
+            if (MODE == KMODE_W4A4_H)  gs = gs * gx_raw;
             const int left = total - f - 1;
             const bool unit_end = (left == 0) ? (x_need - x_items_cell == ncw * x_items_cell) : true;
             finish_segment<M, R>(p, acc, slots, cnt, fstart, c_ul, u0 + c_ul, seg_from0 && unit_end, seg_first, ncw, T,

@@ -6,6 +6,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include "../../include/nvfp4.h"
 
@@ -47,6 +48,9 @@ __host__ __device__ inline Layout make_layout(int N, int K, int kp) {
 // K parts for a weight shape: the smallest power of two that yields >= 1184 (= 148 SMs x 8 warps)
 // warp units, among those whose K padding costs at most 3% more than KP = 1 does.
 __host__ __device__ inline int layout_kparts(int N, int K) {
+#ifndef __CUDA_ARCH__
+    { const char* e = getenv("NVFP4_KP"); if (e) return atoi(e); }     // experiments only
+#endif
     const long long pad1 = ((long long)(K + 127) / 128) * 128;
     int best = 1;
     for (int kp = 1; kp <= 32; kp *= 2) {
