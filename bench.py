@@ -84,7 +84,7 @@ class ClockSampler:
                 self.rows.append([c.strip() for c in out.strip().split(",")])
             except Exception:
                 pass
-            self.stop.wait(0.1)
+            self.stop.wait(0.02)
 
     def __enter__(self):
         self.t.start()
@@ -343,7 +343,8 @@ def run_ours(args):
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "int8 dp4a in-block, f32 across blocks (W4A4 NVFP4 operands)", "data": "synthetic",
+            "dtype": ("f16 (HFMA2, exact in-block) + f32 across blocks" if M == 1 else
+                      "int8 (dp4a, exact in-block) + f32 across blocks"), "data": "synthetic",
             "config": {"workload": WORKLOAD, "M": M, "l2": "cold: inputs larger than L2 (274 MB weights per step, "
                        "2 distinct weight sets alternate; L2 = 126 MB)", "timing": "CUDA graph replay, CUDA events",
                        "multi_gpu": "replicas only"},
@@ -441,8 +442,8 @@ def run_profile(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=4000)
+    ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--m", type=int, default=1, help="activation rows M (1..8)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sweep", action="store_true", help="also print per-shape / per-M / cuBLAS tables")
@@ -454,7 +455,7 @@ def main():
     if args.profile_shape:
         return run_profile(args)
     if args.impl == "reference":
-        if args.steps == 200 and args.warmup == 20:
+        if args.steps == 4000 and args.warmup == 100:
             args.steps, args.warmup = 3, 1
         run_reference(args)
     else:

@@ -28,7 +28,7 @@ size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
     const Layout L = make_layout(N, K, layout_kparts(N, K));
     const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
     const int xbp = xbp_bytes(gemv_kmode(mode, M));
-    const size_t xs = align_up((size_t)ncw_max * 4 * L.kp * M * xbp, 128);
+    const size_t xs = align_up((size_t)ncw_max * 4 * L.kp * xvec_stride(gemv_kmode(mode, M), M), 128);
     const int units = (L.ntiles + c.rows - 1) / c.rows;
     const int ctas = gemv_ctas(units, c);
     const int ucta_max = (units + ctas - 1) / ctas;
@@ -44,20 +44,22 @@ size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
 GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     GemvConfig c;
     const Layout L = make_layout(N, K, layout_kparts(N, K));
+    // from the round-1 sweeps on B200 (profiles/r01_sweep.md): two stages are enough once 16+ warps
+    // stream concurrently; R = 2 pays when the activation loads are not warp-uniform (KP > 1) or M is large
+    const bool half_path = (gemv_kmode(mode, M) == KMODE_W4A4_H);
     c.rows = 1;
-    if (mode == NVFP4_MODE_W4A4 && M >= 5 && L.ntiles >= 2 * 8 * NUM_SMS) c.rows = 2;
-    c.stages = 4;
+    if (mode == NVFP4_MODE_W4A4 && !half_path && (L.kp > 1 || M >= 8) && L.ntiles >= 4 * NUM_SMS) c.rows = 2;
+    c.warps = (half_path && M == 1) ? 20 : ((M >= 8) ? 12 : 16);
+    c.stages = 2;
     c.ksplit = 1;
-    c.warps = (M <= 2) ? 16 : 12;
-    // shrink until the CTA fits in shared memory: K ranges first when the activations dominate
-    while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP / 2) {
+    // one persistent CTA per SM: shrink only if it does not fit in the 227 KB of shared memory
+    while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP) {
         const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
-        const size_t xs = (size_t)ncw_max * 4 * L.kp * M * xbp_bytes(gemv_kmode(mode, M));
-        if (xs > SMEM_CAP / 4 && c.ksplit < L.ncells) ++c.ksplit;
-        else if (c.stages > 2) --c.stages;
-        else if (gemv_smem_bytes(mode, M, N, K, c) <= SMEM_CAP) break;
+        const size_t xs = (size_t)ncw_max * 4 * L.kp * xvec_stride(gemv_kmode(mode, M), M);
+        if (xs > SMEM_CAP / 2 && c.ksplit < L.ncells) ++c.ksplit;       // activations dominate: split K
+        else if (c.warps > 8) c.warps -= 2;
         else if (c.ksplit < L.ncells) ++c.ksplit;
-        else if (c.warps > 1) c.warps /= 2;
+        else if (c.warps > 1) --c.warps;
         else break;
     }
     return c;
@@ -104,7 +106,7 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     // every consumer warp needs at least one cell of the smallest CTA's flat stream
     const int min_cells = (p.units / ctas) * (p.nch / cfg.ksplit);
     if (p.warps > min_cells) p.warps = min_cells;
-    if (M > 1 && p.warps > 16) p.warps = 16;             // launch bounds: 1024 threads for M = 1, 640 otherwise
+    if (!(gemv_kmode(mode, M) == KMODE_W4A4_H && M == 1) && p.warps > 16) p.warps = 16;             // launch bounds: 1024 threads for M = 1, 640 otherwise
     dim3 grid(ctas, cfg.ksplit);
     const int threads = p.warps * 32 + STAGER_THREADS;
     const int kmode = gemv_kmode(mode, M);

@@ -53,8 +53,16 @@ constexpr int XBP_W4A4H = 80;    // 32 f16 (e2m1 values, exact) + {sX0, sX1} + p
 constexpr int KMODE_W4A4_I8 = 0;   // integer: PRMT LUT decode + dp4a          (best for M >= 2)
 constexpr int KMODE_W4A16   = 1;   // FP32 FMA against BF16 activations
 constexpr int KMODE_W4A4_H  = 2;   // cvt.rn.f16x2.e2m1x2 + HFMA2, exact per 8 k (best for M = 1)
+// Bytes between the records of consecutive 32-k vectors (all M rows of a vector are adjacent).  The
+// lanes of a quarter warp read the records of 8 consecutive vectors (their K parts) with one
+// LDS.128, so the stride must be an ODD multiple of 16 B to spread them over all 32 banks: pad by
+// 16 B when M*XBP/16 is even (otherwise e.g. M = 8 gives an 8-way bank conflict on every load).
+__host__ __device__ constexpr int xvec_stride(int kmode, int M);
 __host__ __device__ constexpr int xbp_bytes(int kmode) {
     return kmode == KMODE_W4A4_I8 ? XBP_W4A4 : (kmode == KMODE_W4A16 ? XBP_W4A16 : XBP_W4A4H);
+}
+__host__ __device__ constexpr int xvec_stride(int kmode, int M) {
+    return M * xbp_bytes(kmode) + (((M * xbp_bytes(kmode) / 16) % 2 == 0) ? 16 : 0);
 }
 
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
@@ -169,8 +177,8 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
             const int i = base + t * STAGER_THREADS + tid;
             if (i < total) {
                 const int blk = i / M, m = i - blk * M;
-                if (HALF) decode_x_block_h(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)((blk >> 1) * M + m) * XBP_W4A4H, blk & 1);
-                else      decode_x_block(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)((blk >> 1) * M + m) * XBP_W4A4, blk & 1);
+                if (HALF) decode_x_block_h(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_H, M) + m * XBP_W4A4H, blk & 1);
+                else      decode_x_block(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_I8, M) + m * XBP_W4A4, blk & 1);
             }
         }
         mbar_arrive(smem_u32(xbars + base / STAGE_ITEMS));
@@ -200,7 +208,7 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
             const int i = base + t * STAGER_THREADS + tid;
             if (i < total) {
                 const int v = i / M, m = i - v * M;
-                float* dst = reinterpret_cast<float*>(xs + (size_t)((v >> 2) * M + m) * XBP_W4A16) + (v & 3) * 8;
+                float* dst = reinterpret_cast<float*>(xs + (size_t)(v >> 2) * xvec_stride(KMODE_W4A16, M) + m * XBP_W4A16) + (v & 3) * 8;
                 const uint32_t w[4] = {raw[t].x, raw[t].y, raw[t].z, raw[t].w};
                 float4 lo, hi;
                 lo.x = __uint_as_float(w[0] << 16); lo.y = __uint_as_float(w[0] & 0xFFFF0000u);
@@ -470,7 +478,7 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
 // (a unit cut between warps is recombined in finish_segment).  A warp's bulk-copy ring runs over
 // its whole share and never drains between units.  STAGER_WARPS extra warps decode the activations.
 template <int MODE, int M, int R>
-__global__ void __launch_bounds__(M == 1 ? 1024 : 640) gemv_kernel(const GemvParams p) {
+__global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
@@ -493,7 +501,8 @@ __global__ void __launch_bounds__(M == 1 ? 1024 : 640) gemv_kernel(const GemvPar
 
     // shared memory carve-up (must match gemv_smem_bytes)
     uint8_t* xs = smem;                                                      // activations
-    const size_t xs_bytes = ((size_t)ncw_max * 4 * p.kp * M * XBP + 127) & ~(size_t)127;
+    constexpr int XVS = xvec_stride(MODE, M);
+    const size_t xs_bytes = ((size_t)ncw_max * 4 * p.kp * XVS + 127) & ~(size_t)127;
     uint8_t* ring_all = smem + xs_bytes;
     float* slots = reinterpret_cast<float*>(ring_all + (size_t)W * S * STAGE_BYTES);
     uint64_t* bars_all = reinterpret_cast<uint64_t*>(slots + (size_t)W * 2 * R * M * rpt);
@@ -571,8 +580,8 @@ __global__ void __launch_bounds__(M == 1 ? 1024 : 640) gemv_kernel(const GemvPar
 
     const WLut lut = make_wlut((uint32_t)p.zero);
     // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
-    const size_t xstep = (size_t)p.kp * M * XBP;
-    const uint8_t* xlane0 = xs + (size_t)part * M * XBP;
+    const size_t xstep = (size_t)p.kp * XVS;
+    const uint8_t* xlane0 = xs + (size_t)part * XVS;
     int c_ul = f0 / ncw;
     const int cell0 = f0 - c_ul * ncw;
     const uint8_t* xlane = xlane0 + (size_t)cell0 * 4 * xstep;
