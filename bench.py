@@ -439,6 +439,31 @@ def run_profile(args):
     print(json.dumps({"profile_shape": args.profile_shape, "M": args.m, "mode": args.mode, "launches": n}))
 
 
+def run_chain(args):
+    """BASELINE.json configs[4]: 64 layers x 4 projections (+ quantizers + SiLU*mul), distinct weights per
+    layer (17.5 GB, every call HBM-cold), one CUDA graph per M; prints one JSON line per M."""
+    import torch
+    from paper_2606_13233_b200.chain import DecodeChain
+    peak, _ = measured_peak()
+    for M in (1, 2, 4, 8):
+        ch = DecodeChain(layers=args.layers, M=M)
+        ch.set_input(torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16))
+        ch.step()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            ch.step()
+        ms = time_graph(torch, g, 20, 3)
+        finite = bool(torch.isfinite(ch.h.float()).all())
+        wb = ch.weight_bytes()
+        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "ms_per_token": round(ms, 4),
+                          "us_per_layer": round(ms * 1e3 / args.layers, 2), "weight_gb": round(wb / 1e9, 2),
+                          "gbs": round(wb / ms / 1e6, 1), "frac_of_copy_peak": round(wb / ms / 1e6 / peak, 3),
+                          "launches": ch.launches_per_step, "finite": finite}), flush=True)
+        del ch, g
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -451,9 +476,13 @@ def main():
     ap.add_argument("--profile-shape", default=None, help="qkv|o|gate_up|down|all: plain stream launches of "
                     "quantize_act + gemv on that shape only (for ncu); prints a short JSON line")
     ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16"])
+    ap.add_argument("--chain", action="store_true", help="configs[4]: decode-step projection chain, M = 1,2,4,8")
+    ap.add_argument("--layers", type=int, default=64)
     args = ap.parse_args()
     if args.profile_shape:
         return run_profile(args)
+    if args.chain:
+        return run_chain(args)
     if args.impl == "reference":
         if args.steps == 4000 and args.warmup == 100:
             args.steps, args.warmup = 3, 1

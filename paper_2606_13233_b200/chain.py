@@ -1,0 +1,76 @@
+"""Decode-step projection chain of BASELINE.json configs[4]: L layers x {QKV, O, gate_up, down}, W4A4,
+distinct NVFP4 weights per layer, `nvfp4_quantize_act` before every projection and SiLU*mul between
+gate_up and down, all enqueued on the current stream (capture it in a CUDA graph to time it).
+
+Data flow (R11, R12; there is no attention here, this isolates the projections):
+    h [M,H] -> Q -> QKV -> first `o_in` columns -> Q -> O -> Q -> gate_up -> SiLU*mul -> Q -> down -> h'
+Product code: uses only the ctypes binding (no oracle, no torch math on the path).
+"""
+from __future__ import annotations
+
+import math
+
+import torch
+
+from . import binding as B
+from . import inputs
+
+QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
+
+
+class DecodeChain:
+    def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda"):
+        d = dict(QWEN3_32B_DIMS if dims is None else dims)
+        self.M, self.layers, self.d = M, layers, d
+        H, QKV, OIN, I = d["hidden"], d["qkv"], d["o_in"], d["inter"]
+        self.shapes = (("qkv", QKV, H), ("o", H, OIN), ("gate_up", 2 * I, H), ("down", H, I))
+        self.w = []                                   # per layer: list of (blob, gW tensor, N, K)
+        self.canon = []                               # canonical bytes kept only when asked (tests)
+        for l in range(layers):
+            row = []
+            for sid, (name, N, K) in enumerate(self.shapes):
+                codes, scales, _ = inputs.make_nvfp4_weight_device(N, K, seed=seed * 1000 + l, shape_id=sid + 1,
+                                                                   device=device)
+                g = 1.0 / (557.0 * math.sqrt(K))       # keeps activations O(1) through the chain
+                row.append((B.nvfp4_repack_weight(codes, scales),
+                            torch.tensor([g], dtype=torch.float32, device=device), N, K))
+                del codes, scales
+            self.w.append(row)
+        bf, u8 = torch.bfloat16, torch.uint8
+        self.h = torch.zeros((M, H), dtype=bf, device=device)            # layer input / output
+        self.y_qkv = torch.empty((M, QKV), dtype=bf, device=device)
+        self.y_o = torch.empty((M, H), dtype=bf, device=device)
+        self.y_gu = torch.empty((M, 2 * I), dtype=bf, device=device)
+        self.act = torch.empty((M, I), dtype=bf, device=device)
+        kmax = max(K for _, _, K in self.shapes)
+        self.xc = torch.empty((M, kmax // 2), dtype=u8, device=device)   # reused NVFP4 activation buffers
+        self.xs = torch.empty((M, kmax // 16), dtype=u8, device=device)
+        self.gx = torch.zeros(1, dtype=torch.float32, device=device)
+        self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
+        self.launches_per_step = layers * 9
+
+    def set_input(self, h_bf16):
+        self.h.copy_(h_bf16)
+
+    def _proj(self, l, i, x, y):
+        blob, gw, N, K = self.w[l][i]
+        xc = self.xc.view(-1)[: self.M * (K // 2)].view(self.M, K // 2)
+        xs = self.xs.view(-1)[: self.M * (K // 16)].view(self.M, K // 16)
+        B.nvfp4_quantize_act(x, xc, xs, self.gx)
+        B.nvfp4_gemv(B.MODE_W4A4, blob, gw, N, K, xc, xs, self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])
+
+    def step(self, taps=None):
+        """enqueue the whole chain once; `taps` (tests) collects (layer, name, input clone, output clone)."""
+        d = self.d
+        for l in range(self.layers):
+            stages = (("qkv", self.h, self.y_qkv), ("o", self.y_qkv[:, : d["o_in"]], self.y_o),
+                      ("gate_up", self.y_o, self.y_gu), ("down", self.act, self.h))
+            for i, (name, x, y) in enumerate(stages):
+                if name == "down":
+                    B.nvfp4_silu_mul(self.y_gu, self.act)
+                self._proj(l, i, x, y)
+                if taps is not None:
+                    taps.append((l, name, x.clone(), y.clone()))
+
+    def weight_bytes(self):
+        return self.layers * sum(N * K * 9 // 16 for _, N, K in self.shapes)

@@ -1,0 +1,48 @@
+"""GPU: the decode-step projection chain (configs[4] data flow) -- every projection of every layer
+is checked against the oracle run on that projection's own downloaded input and unpacked weights."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nvfp4_oracle as orc
+from paper_2606_13233_b200 import inputs
+import _gpu_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("M", [1, 4])
+def test_chain_small_dims_every_stage(M):
+    from paper_2606_13233_b200 import binding as B
+    from paper_2606_13233_b200.chain import DecodeChain
+    dims = dict(hidden=256, qkv=512, o_in=384, inter=512)
+    ch = DecodeChain(layers=3, M=M, dims=dims, seed=5)
+    ch.set_input(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77)))
+    taps = []
+    ch.step(taps)
+    torch.cuda.synchronize()
+    assert len(taps) == 12
+    for l, name, x, y in taps:
+        i = [s[0] for s in ch.shapes].index(name)
+        blob, gw, N, K = ch.w[l][i]
+        wc, ws = B.nvfp4_unpack_weight(blob, N, K)
+        xf = orc.bf16_bits_to_f32(U.host_bf16_bits(x.contiguous()))
+        assert np.all(np.isfinite(xf))
+        oxc, oxs, ogx = orc.quantize(xf)
+        Y, A = orc.gemv_w4a4(U.host_u8(wc), U.host_u8(ws), np.float32(gw.item()), oxc, oxs, ogx)
+        U.check_gemv(U.host_y_f64(y), Y, A, f"layer {l} {name}", bf16_slack=True)
+        if name == "gate_up":       # the glue that feeds `down`
+            want = orc.silu_mul(orc.bf16_bits_to_f32(U.host_bf16_bits(y)))
+            nxt = [t for t in taps if t[0] == l and t[1] == "down"][0][2]
+            got = U.host_y_f64(nxt)
+            assert np.all(np.abs(got - want) <= np.maximum(np.abs(want), 2.0 ** -120) * 2.0 ** -7)
+    # graph replay gives the same bits as the eager run (stateless calls, clean workspaces)
+    h0 = U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77))
+    ch.set_input(h0); ch.step(); torch.cuda.synchronize()
+    ref = ch.h.clone()
+    g = torch.cuda.CUDAGraph()
+    ch.set_input(h0)
+    with torch.cuda.graph(g):
+        ch.step()
+    ch.set_input(h0); g.replay(); torch.cuda.synchronize()
+    assert torch.equal(ch.h, ref)
