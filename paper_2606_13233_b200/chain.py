@@ -72,5 +72,27 @@ class DecodeChain:
                 if taps is not None:
                     taps.append((l, name, x.clone(), y.clone()))
 
+    def calibrate(self, h_bf16):
+        """set-up only (synthetic weights, not part of the timed path): walk the chain once and rescale every
+        projection's global weight scale so that its output has unit RMS -- keeps activations O(1) through
+        all layers whatever M and the input are."""
+        d = self.d
+        self.h.copy_(h_bf16)
+        for l in range(self.layers):
+            stages = (("qkv", self.h, self.y_qkv), ("o", self.y_qkv[:, : d["o_in"]], self.y_o),
+                      ("gate_up", self.y_o, self.y_gu), ("down", self.act, self.h))
+            for i, (name, x, y) in enumerate(stages):
+                if name == "down":
+                    B.nvfp4_silu_mul(self.y_gu, self.act)
+                self._proj(l, i, x, y)
+                rms = float(y.float().pow(2).mean().sqrt())
+                if rms > 0 and math.isfinite(rms):
+                    self.w[l][i][1].div_(rms)
+                else:
+                    self.w[l][i][1].mul_(2.0 ** -20 if not math.isfinite(rms) else 1.0)
+                self._proj(l, i, x, y)
+        torch.cuda.synchronize()
+        self.h.copy_(h_bf16)
+
     def weight_bytes(self):
         return self.layers * sum(N * K * 9 // 16 for _, N, K in self.shapes)

@@ -17,7 +17,7 @@ def test_chain_small_dims_every_stage(M):
     from paper_2606_13233_b200.chain import DecodeChain
     dims = dict(hidden=256, qkv=512, o_in=384, inter=512)
     ch = DecodeChain(layers=3, M=M, dims=dims, seed=5)
-    ch.set_input(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77)))
+    ch.calibrate(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77)))
     taps = []
     ch.step(taps)
     torch.cuda.synchronize()
@@ -32,6 +32,7 @@ def test_chain_small_dims_every_stage(M):
         Y, A = orc.gemv_w4a4(U.host_u8(wc), U.host_u8(ws), np.float32(gw.item()), oxc, oxs, ogx)
         U.check_gemv(U.host_y_f64(y), Y, A, f"layer {l} {name}", bf16_slack=True)
         if name == "gate_up":       # the glue that feeds `down`
+            assert np.all(np.isfinite(U.host_y_f64(y)))
             want = orc.silu_mul(orc.bf16_bits_to_f32(U.host_bf16_bits(y)))
             nxt = [t for t in taps if t[0] == l and t[1] == "down"][0][2]
             got = U.host_y_f64(nxt)
