@@ -14,8 +14,11 @@ static cudaError_t launch_one(const GemvParams& p, dim3 grid, int threads, size_
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    gemv_kernel<MODE, M, R><<<grid, threads, smem, st>>>(p);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1] = {pdl_attribute()};
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, gemv_kernel<MODE, M, R>, p);
 }
 
 template <int MODE, int M>

@@ -520,6 +520,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640)
 
     if (warp >= W) {                                                        // ---- stager warps ----
         const int tid = threadIdx.x - W * 32;
+        pdl_wait();                                   // the activations come from the previous kernel
         if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, tid, xbars);
         else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, tid, xbars);
         return;
@@ -568,6 +569,9 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640)
         const int npre = total < S ? total : S;
         for (int i = 0; i < npre; ++i) issue();
     }
+    // the weight stream is under way; everything below touches data of the previous kernel
+    pdl_wait();
+    pdl_launch_dependents();
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
     const float gx_raw = (MODE == KMODE_W4A16) ? 1.0f : __ldg(p.x_gscale);

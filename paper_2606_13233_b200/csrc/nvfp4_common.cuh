@@ -109,6 +109,16 @@ __device__ __forceinline__ uint16_t float_to_bf16_rn(float f) {
     return r;
 }
 
+// ---- programmatic dependent launch (PDL) --------------------------------------------------
+// Every kernel of the path is launched with cudaLaunchAttributeProgrammaticStreamSerialization, so
+// it may start while its stream predecessor is still running.  pdl_wait() blocks until the
+// predecessor grid has completed and its writes are visible: it must precede every access to
+// memory the predecessor may write or read-before-overwrite (activations, outputs, workspace).
+// Work on constant data (the repacked weights) is issued BEFORE it, which is the point.
+// pdl_launch_dependents() is called only AFTER pdl_wait(), so at most two consecutive kernels overlap.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- mbarrier / bulk-copy (TMA) wrappers ------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return (uint32_t)__cvta_generic_to_shared(p);

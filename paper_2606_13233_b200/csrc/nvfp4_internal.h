@@ -14,6 +14,14 @@ struct GemvConfig {
     int ksplit;   // number of K ranges (grid.y); > 1 -> partials through the workspace
 };
 
+// launch attribute that lets a kernel start before its stream predecessor has finished (PDL)
+inline cudaLaunchAttribute pdl_attribute() {
+    cudaLaunchAttribute a = {};
+    a.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    a.val.programmaticStreamSerializationAllowed = 1;
+    return a;
+}
+
 cudaError_t launch_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* codes, uint8_t* scales,
                                 float* gscale, int gscale_mode, cudaStream_t st);
 

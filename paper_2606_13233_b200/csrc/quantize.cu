@@ -65,6 +65,8 @@ quantize_act_kernel(const uint16_t* __restrict__ x, int M, int K, int64_t ldx,
     const int NB = M * kb_per_row;
     const int nthreads = gridDim.x * blockDim.x;
     const int gtid = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_wait();                                       // X is the previous kernel's output
+    pdl_launch_dependents();                          // the GEMV may start streaming its weights now
 
     uint4 va[BPT], vb[BPT];
     uint32_t ab[BPT];
@@ -170,13 +172,14 @@ static cudaError_t launch_cluster(int nctas, int threads, cudaStream_t st, const
     cfg.gridDim = dim3(nctas);
     cfg.blockDim = dim3(threads);
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
+    attr[1] = pdl_attribute();
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = nctas;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = 2;
     return cudaLaunchKernelEx(&cfg, quantize_act_kernel<BPT, DYN>, x, M, K, ldx, codes, scales, gscale);
 }
 
