@@ -88,9 +88,9 @@ int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx,
 /*
  * Offline weight repack, step a0.  The blob holds exactly the information of the canonical
  * (codes, scales) pair, permuted into the order the GEMV's 128-bit loads consume
- * (2304-byte cells of 32/KP rows x 128*KP k, where the number of K
+ * (4608-byte cells of 32/KP rows x 256*KP k, where the number of K
  * parts KP in {1,2,4,..,32} is a fixed function of (N, K)); rows are padded to a multiple of
- * 32/KP and K to a multiple of 128*KP with zero codes / zero scales (<= 3% extra for K).  nvfp4_repacked_bytes returns 0 for an unsupported shape.
+ * 32/KP and K to a multiple of 256*KP with zero codes / zero scales (<= 3% extra for K).  nvfp4_repacked_bytes returns 0 for an unsupported shape.
  *   codes  [device] uint8 [N, K/2];  scales [device] uint8 [N, K/16];  blob_out [device].
  * nvfp4_unpack_weight is the exact inverse (blob -> canonical, byte-identical).
  */

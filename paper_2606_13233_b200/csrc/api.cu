@@ -104,7 +104,7 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
 }
 
 int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages) {
-    if (ksplit < 0 || ksplit > 64 || warps < 0 || warps > 28 || stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
+    if (ksplit < 0 || ksplit > 64 || warps < 0 || warps > 20 || stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
     if (!(rows == 0 || rows == 1 || rows == 2 || rows == 4)) return NVFP4_ERR_INVALID_ARG;
     g_override.ksplit = ksplit; g_override.warps = warps; g_override.rows = rows; g_override.stages = stages;
     return NVFP4_OK;

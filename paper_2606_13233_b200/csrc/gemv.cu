@@ -28,14 +28,14 @@ size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
     const Layout L = make_layout(N, K, layout_kparts(N, K));
     const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
     const int xbp = xbp_bytes(gemv_kmode(mode, M));
-    const size_t xs = align_up((size_t)ncw_max * 4 * L.kp * xvec_stride(gemv_kmode(mode, M), M), 128);
+    const size_t xs = align_up((size_t)ncw_max * CELL_VECS * L.kp * xvec_stride(gemv_kmode(mode, M), M), 128);
     const int units = (L.ntiles + c.rows - 1) / c.rows;
     const int ctas = gemv_ctas(units, c);
     const int ucta_max = (units + ctas - 1) / ctas;
     return xs + (size_t)c.warps * c.stages * c.rows * CELL_BYTES             // rings
          + (size_t)c.warps * 2 * c.rows * M * L.rpt * sizeof(float)          // segment slots
          + (size_t)c.warps * c.stages * 8                                    // ring mbarriers
-         + ((size_t)ncw_max * L.kp * M * 16 / STAGE_ITEMS + 2) * 8          // staging-batch mbarriers
+         + ((size_t)ncw_max * L.kp * M * 4 * CELL_VECS / STAGE_ITEMS + 2) * 8          // staging-batch mbarriers
          + (size_t)(ucta_max + c.warps + 4) * sizeof(int);                   // unit counters + share starts
 }
 
@@ -49,13 +49,13 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     const bool half_path = (gemv_kmode(mode, M) == KMODE_W4A4_H);
     c.rows = 1;
     if (mode == NVFP4_MODE_W4A4 && !half_path && (L.kp > 1 || M >= 8) && L.ntiles >= 4 * NUM_SMS) c.rows = 2;
-    c.warps = (half_path && M == 1) ? 20 : ((M >= 8) ? 12 : 16);
+    c.warps = (M >= 8) ? 12 : 16;
     c.stages = 2;
     c.ksplit = 1;
     // one persistent CTA per SM: shrink only if it does not fit in the 227 KB of shared memory
     while (gemv_smem_bytes(mode, M, N, K, c) > SMEM_CAP) {
         const int ncw_max = (L.ncells + c.ksplit - 1) / c.ksplit;
-        const size_t xs = (size_t)ncw_max * 4 * L.kp * xvec_stride(gemv_kmode(mode, M), M);
+        const size_t xs = (size_t)ncw_max * CELL_VECS * L.kp * xvec_stride(gemv_kmode(mode, M), M);
         if (xs > SMEM_CAP / 2 && c.ksplit < L.ncells) ++c.ksplit;       // activations dominate: split K
         else if (c.warps > 8) c.warps -= 2;
         else if (c.ksplit < L.ncells) ++c.ksplit;

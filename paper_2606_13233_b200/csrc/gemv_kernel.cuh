@@ -153,9 +153,9 @@ __device__ __forceinline__ void decode_x_block_h(uint2 cw, float sx, uint8_t* ba
 template <int M, bool HALF>
 __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
                                              uint64_t* xbars) {
-    const int nblk = ncw * 8 * p.kp;                             // 16-blocks in the range
+    const int nblk = ncw * 2 * CELL_VECS * p.kp;                 // 16-blocks in the range
     const int kb_total = p.K >> 4;
-    const int kb0 = c0 * 8 * p.kp;
+    const int kb0 = c0 * 2 * CELL_VECS * p.kp;
     const uint8_t* xc = static_cast<const uint8_t*>(p.x);
     const int total = nblk * M;
     for (int base = 0; base < total; base += STAGER_THREADS * STAGE_BATCH) {
@@ -189,10 +189,10 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
 template <int M>
 __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
                                               uint64_t* xbars) {
-    const int nvec = ncw * 16 * p.kp;                            // 8-element vectors per row in the range
+    const int nvec = ncw * 4 * CELL_VECS * p.kp;                 // 8-element vectors per row in the range
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
     const int total = nvec * M;
-    const int k_base = c0 * 128 * p.kp;
+    const int k_base = c0 * 32 * CELL_VECS * p.kp;
     for (int base = 0; base < total; base += STAGER_THREADS * STAGE_BATCH) {
         uint4 raw[STAGE_BATCH];
 #pragma unroll
@@ -478,7 +478,7 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
 // (a unit cut between warps is recombined in finish_segment).  A warp's bulk-copy ring runs over
 // its whole share and never drains between units.  STAGER_WARPS extra warps decode the activations.
 template <int MODE, int M, int R>
-__global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640) gemv_kernel(const GemvParams p) {
+__global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
@@ -502,11 +502,11 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640)
     // shared memory carve-up (must match gemv_smem_bytes)
     uint8_t* xs = smem;                                                      // activations
     constexpr int XVS = xvec_stride(MODE, M);
-    const size_t xs_bytes = ((size_t)ncw_max * 4 * p.kp * XVS + 127) & ~(size_t)127;
+    const size_t xs_bytes = ((size_t)ncw_max * CELL_VECS * p.kp * XVS + 127) & ~(size_t)127;
     uint8_t* ring_all = smem + xs_bytes;
     float* slots = reinterpret_cast<float*>(ring_all + (size_t)W * S * STAGE_BYTES);
     uint64_t* bars_all = reinterpret_cast<uint64_t*>(slots + (size_t)W * 2 * R * M * rpt);
-    const int xitems = ncw_max * p.kp * M * ((MODE == KMODE_W4A16) ? 16 : 8);  // staging work items (upper bound)
+    const int xitems = ncw_max * p.kp * M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2);  // staging items (upper bound)
     const int nxb = (xitems + STAGE_ITEMS - 1) / STAGE_ITEMS;
     uint64_t* xbars = bars_all + W * S;
     int* cnt = reinterpret_cast<int*>(xbars + nxb);
@@ -588,7 +588,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640)
     const uint8_t* xlane0 = xs + (size_t)part * XVS;
     int c_ul = f0 / ncw;
     const int cell0 = f0 - c_ul * ncw;
-    const uint8_t* xlane = xlane0 + (size_t)cell0 * 4 * xstep;
+    const uint8_t* xlane = xlane0 + (size_t)cell0 * CELL_VECS * xstep;
     // loop state kept incremental (no per-iteration index arithmetic): consumer stage pointer and
     // barrier, cells left in the current segment, staging items this lane's next cell depends on
     const uint8_t* st = ring;
@@ -597,7 +597,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640)
     uint32_t phase = 0;
     int seg_left = (ncw - cell0) < total ? (ncw - cell0) : total;           // cells until the segment ends
     bool seg_first = true, seg_from0 = (cell0 == 0);
-    constexpr int ITEMS_PER_CELL_KP = M * ((MODE == KMODE_W4A16) ? 16 : 8); // staging items per cell and K part
+    constexpr int ITEMS_PER_CELL_KP = M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2); // staging items per cell and K part
     const int x_items_cell = p.kp * ITEMS_PER_CELL_KP;
     int x_need = (cell0 + 1) * x_items_cell;                                // items that must be staged
     int x_have = 0;                                                         // items known to be staged
@@ -607,29 +607,32 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 1024 : 640)
         while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += STAGE_ITEMS; }
         mbar_wait(bar, phase);
 
-        float sw[R][8];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * 8);
-            const float2 f0s = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
-            const float2 f1s = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
-            const float2 f2s = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
-            const float2 f3s = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
-            sw[r][0] = f0s.x; sw[r][1] = f0s.y; sw[r][2] = f1s.x; sw[r][3] = f1s.y;
-            sw[r][4] = f2s.x; sw[r][5] = f2s.y; sw[r][6] = f3s.x; sw[r][7] = f3s.y;
+        for (int hc = 0; hc < CELL_VECS / 4; ++hc) {                       // half cells: 8 scales, 4 vectors
+            float sw[R][8];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * (2 * CELL_VECS) + hc * 8);
+                const float2 f0s = e4m3x2_to_float2((uint16_t)(sc.x & 0xFFFFu));
+                const float2 f1s = e4m3x2_to_float2((uint16_t)(sc.x >> 16));
+                const float2 f2s = e4m3x2_to_float2((uint16_t)(sc.y & 0xFFFFu));
+                const float2 f3s = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
+                sw[r][0] = f0s.x; sw[r][1] = f0s.y; sw[r][2] = f1s.x; sw[r][3] = f1s.y;
+                sw[r][4] = f2s.x; sw[r][5] = f2s.y; sw[r][6] = f3s.x; sw[r][7] = f3s.y;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {                                  // 32-k vectors of this lane
+                uint4 wv[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + (hc * 4 + j) * 512 + lane * 16);
+                const uint8_t* xbp = xlane + (size_t)(hc * 4 + j) * xstep;
+                if (MODE == KMODE_W4A4_I8)     block_pair_w4a4<M, R>(lut, wv, xbp, sw, j, acc);
+                else if (MODE == KMODE_W4A4_H) block_pair_w4a4_h<M, R>(wv, xbp, sw, j, acc);
+                else                           block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
+            }
         }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {                                      // four 32-k vectors of this lane
-            uint4 wv[R];
-#pragma unroll
-            for (int r = 0; r < R; ++r)
-                wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + j * 512 + lane * 16);
-            const uint8_t* xbp = xlane + (size_t)j * xstep;
-            if (MODE == KMODE_W4A4_I8)     block_pair_w4a4<M, R>(lut, wv, xbp, sw, j, acc);
-            else if (MODE == KMODE_W4A4_H) block_pair_w4a4_h<M, R>(wv, xbp, sw, j, acc);
-            else                           block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
-        }
-        xlane += 4 * xstep;
+        xlane += CELL_VECS * xstep;
         x_need += x_items_cell;
 
         // every lane has read the stage -> lane 0 requests the next cell of the share into it

@@ -20,26 +20,27 @@ namespace nvfp4 {
 // A lane of the GEMV owns (row r, K part p): lane = r*KP + p, KP = 2^i K parts per row inside a
 // warp (chosen per weight shape by layout_kparts, so that N*KP/32 independent warp units fill
 // the 148 SMs without any cross-warp or cross-CTA reduction).  A "cell" is what one warp consumes
-// in four 128-bit loads per lane: 32/KP weight rows x 128*KP consecutive k:
-//   bytes [0,2048)    codes:  vector j (0..3), lane (r,p) -> 16 B = the 32 k starting at
+// in CELL_VECS = 8 128-bit loads per lane: 32/KP weight rows x 256*KP consecutive k:
+//   bytes [0,4096)    codes:  vector j (0..7), lane (r,p) -> 16 B = the 32 k starting at
 //                             cell_k0 + (j*KP + p)*32 of row tile_row0 + r
-//   bytes [2048,2304) scales: lane (r,p) -> 8 B = the E4M3 scales of those 4 x 2 blocks (j-major)
-// Blob = cells in [tile = n/(32/KP)][cell = k/(128*KP)] order, so one warp streams a contiguous run.
-constexpr int CELL_CODES  = 2048;
-constexpr int CELL_SCALES = 256;
-constexpr int CELL_BYTES  = CELL_CODES + CELL_SCALES;  // 2304 = 0.5625 B per weight
+//   bytes [4096,4608) scales: lane (r,p) -> 16 B = the E4M3 scales of those 8 x 2 blocks (j-major)
+// Blob = cells in [tile = n/(32/KP)][cell = k/(256*KP)] order, so one warp streams a contiguous run.
+constexpr int CELL_VECS   = 8;                          // 128-bit code vectors per lane and cell
+constexpr int CELL_CODES  = CELL_VECS * 512;            // 4096
+constexpr int CELL_SCALES = CELL_VECS * 64;             // 512
+constexpr int CELL_BYTES  = CELL_CODES + CELL_SCALES;   // 4608 = 0.5625 B per weight
 
 struct Layout {
     int kp;         // K parts per row inside a warp (1, 2, 4, 8, 16 or 32)
     int rpt;        // weight rows per tile = 32 / kp
-    int cell_k;     // k per cell = 128 * kp
+    int cell_k;     // k per cell = 32 * CELL_VECS * kp
     int ntiles;     // ceil(N / rpt)
     int ncells;     // ceil(K / cell_k)
 };
 
 __host__ __device__ inline Layout make_layout(int N, int K, int kp) {
     Layout L;
-    L.kp = kp; L.rpt = 32 / kp; L.cell_k = 128 * kp;
+    L.kp = kp; L.rpt = 32 / kp; L.cell_k = 32 * CELL_VECS * kp;
     L.ntiles = (N + L.rpt - 1) / L.rpt;
     L.ncells = (K + L.cell_k - 1) / L.cell_k;
     return L;
@@ -51,10 +52,11 @@ __host__ __device__ inline int layout_kparts(int N, int K) {
 #ifndef __CUDA_ARCH__
     { const char* e = getenv("NVFP4_KP"); if (e) return atoi(e); }     // experiments only
 #endif
-    const long long pad1 = ((long long)(K + 127) / 128) * 128;
+    const long long ck1 = 32 * CELL_VECS;
+    const long long pad1 = ((K + ck1 - 1) / ck1) * ck1;
     int best = 1;
     for (int kp = 1; kp <= 32; kp *= 2) {
-        const long long ck = 128LL * kp;
+        const long long ck = ck1 * kp;
         const long long padk = ((K + ck - 1) / ck) * ck;
         if (padk * 100 > pad1 * 103) break;
         best = kp;

@@ -10,7 +10,7 @@ namespace nvfp4 {
 struct GemvConfig {
     int warps;    // warps per CTA, each owns `rows` row tiles (32 rows each) -> no cross-warp reduce
     int rows;     // R: row tiles (32/KP rows each) per warp (1, 2 or 4)
-    int stages;   // depth of each warp's private bulk-copy ring (cells of 2304 B per tile)
+    int stages;   // depth of each warp's private bulk-copy ring (cells of 4608 B per tile)
     int ksplit;   // number of K ranges (grid.y); > 1 -> partials through the workspace
 };
 

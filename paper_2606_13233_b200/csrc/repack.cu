@@ -1,5 +1,5 @@
 // repack.cu -- offline weight repack (step a0) and its exact inverse.  Pure byte permutation:
-// canonical codes[N,K/2] + scales[N,K/16]  <->  blob of 2304-byte cells (nvfp4_common.cuh; the
+// canonical codes[N,K/2] + scales[N,K/16]  <->  blob of 4608-byte cells (nvfp4_common.cuh; the
 // K-part count of the layout is a function of (N, K) only).
 // Padding rows (n >= N) and padding k (k >= K) are zero codes / zero scales.
 #include "nvfp4_common.cuh"
@@ -7,21 +7,22 @@
 
 namespace nvfp4 {
 
-// one thread per 16-byte code vector of the blob, one per 8-byte scale group
+// one thread per 16-byte code vector of the blob, one per 16-byte scale group
 template <bool TO_BLOB>
 __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes, uint8_t* __restrict__ scales,
                                                      int N, int K, Layout L, uint8_t* __restrict__ blob) {
     const int64_t ncells = (int64_t)L.ntiles * L.ncells;
-    const int64_t nvec = ncells * (128 + 32);               // 128 code vectors + 32 scale groups per cell
+    constexpr int EPC = CELL_VECS * 32 + 32;                // code vectors + scale groups per cell
+    const int64_t nvec = ncells * EPC;
     const int64_t rowb = K / 2, rows = K / 16;
     for (int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t cell = v / 160;
-        const int e = (int)(v - cell * 160);
+        const int64_t cell = v / EPC;
+        const int e = (int)(v - cell * EPC);
         const int tile = (int)(cell / L.ncells), ci = (int)(cell - (int64_t)tile * L.ncells);
         uint8_t* cellp = blob + cell * CELL_BYTES;
         const int lane = e & 31;
         const int n = tile * L.rpt + lane / L.kp, part = lane % L.kp;
-        if (e < 128) {
+        if (e < CELL_VECS * 32) {
             const int j = e >> 5;
             const int64_t k0 = (int64_t)ci * L.cell_k + (int64_t)(j * L.kp + part) * 32;
             const int64_t b0 = k0 / 2;                          // byte offset inside the canonical row
@@ -32,8 +33,8 @@ __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes
                 else if (valid) codes[(int64_t)n * rowb + b0 + i] = bp[i];
             }
         } else {
-            uint8_t* sp = cellp + CELL_CODES + lane * 8;
-            for (int i = 0; i < 8; ++i) {
+            uint8_t* sp = cellp + CELL_CODES + lane * (2 * CELL_VECS);
+            for (int i = 0; i < 2 * CELL_VECS; ++i) {
                 const int j = i >> 1;
                 const int64_t s0 = ((int64_t)ci * L.cell_k + (int64_t)(j * L.kp + part) * 32) / 16 + (i & 1);
                 const bool valid = (n < N) && (s0 < rows);
@@ -45,7 +46,7 @@ __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes
 }
 
 static int repack_grid(const Layout& L) {
-    const int64_t nvec = (int64_t)L.ntiles * L.ncells * 160;
+    const int64_t nvec = (int64_t)L.ntiles * L.ncells * (CELL_VECS * 32 + 32);
     int64_t g = (nvec + 255) / 256;
     if (g > 148 * 32) g = 148 * 32;
     return (int)g;
