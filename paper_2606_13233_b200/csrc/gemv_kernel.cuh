@@ -319,6 +319,23 @@ __device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const ui
     }
 }
 
+// W4A16: weights to FP32 pairs (F2FP.E2M1 + two f16->f32), packed FP32 FMA (fma.rn.f32x2: two MACs per
+// instruction) against FP32 copies of the BF16 activations; two 4-deep chains per 16-block.
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ float2 unpack2(uint64_t v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
 template <int M, int R>
 __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
                                                  int j, float (&acc)[R][M]) {
@@ -327,26 +344,24 @@ __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uin
         const uint32_t ww[4] = {wv[r].x, wv[r].y, wv[r].z, wv[r].w};
 #pragma unroll
         for (int h = 0; h < 2; ++h) {                                      // the two 16-blocks
-            float wf[16];
+            uint64_t wp[8];
 #pragma unroll
             for (int q = 0; q < 2; ++q)
 #pragma unroll
                 for (int b = 0; b < 4; ++b) {
-                    const uint32_t h2 = e2m1x2_to_f16x2((ww[h * 2 + q] >> (8 * b)) & 0xFFu);
-                    asm("{.reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi;}"
-                        : "=f"(wf[q * 8 + b * 2]), "=f"(wf[q * 8 + b * 2 + 1]) : "r"(h2));
+                    const float2 f = h2_to_float2(e2m1x2_to_f16x2((ww[h * 2 + q] >> (8 * b)) & 0xFFu));
+                    wp[q * 4 + b] = pack2(f.x, f.y);
                 }
 #pragma unroll
             for (int m = 0; m < M; ++m) {
-                const float4* xf = reinterpret_cast<const float4*>(xbp + m * XBP_W4A16) + h * 4;
-                float da = 0.f, db = 0.f;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const float4 x = xf[q];
-                    da = fmaf(wf[q * 4 + 0], x.x, da); db = fmaf(wf[q * 4 + 1], x.y, db);
-                    da = fmaf(wf[q * 4 + 2], x.z, da); db = fmaf(wf[q * 4 + 3], x.w, db);
-                }
-                acc[r][m] = fmaf(da + db, sw[r][2 * j + h], acc[r][m]);
+                const ulonglong2* xp = reinterpret_cast<const ulonglong2*>(xbp + m * XBP_W4A16) + h * 4;
+                const ulonglong2 x0 = xp[0], x1 = xp[1], x2 = xp[2], x3 = xp[3];
+                uint64_t da = ffma2(wp[0], x0.x, 0ull), db = ffma2(wp[4], x2.x, 0ull);
+                da = ffma2(wp[1], x0.y, da); db = ffma2(wp[5], x2.y, db);
+                da = ffma2(wp[2], x1.x, da); db = ffma2(wp[6], x3.x, db);
+                da = ffma2(wp[3], x1.y, da); db = ffma2(wp[7], x3.y, db);
+                const float2 fa = unpack2(da), fb = unpack2(db);
+                acc[r][m] = fmaf((fa.x + fa.y) + (fb.x + fb.y), sw[r][2 * j + h], acc[r][m]);
             }
         }
     }
