@@ -49,7 +49,7 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     const bool half_path = (gemv_kmode(mode, M) == KMODE_W4A4_H);
     c.rows = 1;
     if (mode == NVFP4_MODE_W4A4 && !half_path && (L.kp > 1 || M >= 8) && L.ntiles >= 4 * NUM_SMS) c.rows = 2;
-    c.warps = (M >= 8) ? 12 : 16;
+    c.warps = (M >= 8 || half_path) ? 12 : 16;
     c.stages = 2;
     c.ksplit = 1;
     // one persistent CTA per SM: shrink only if it does not fit in the 227 KB of shared memory

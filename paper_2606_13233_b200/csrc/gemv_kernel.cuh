@@ -282,6 +282,13 @@ __device__ __forceinline__ float2 h2_to_float2(uint32_t h2) {
         : "=f"(r.x), "=f"(r.y) : "r"(h2));
     return r;
 }
+// lo + hi of a half2 in FP32: one f16->f32 conversion and one mixed-precision add (SASS FHADD)
+__device__ __forceinline__ float h2_sum_f32(uint32_t h2) {
+    float r;
+    asm("{.reg .b16 lo, hi; .reg .f32 t; mov.b32 {lo, hi}, %1; cvt.f32.f16 t, lo; add.rn.f32.f16 %0, hi, t;}"
+        : "=f"(r) : "r"(h2));
+    return r;
+}
 template <int M, int R>
 __device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
                                                   int j, float (&acc)[R][M]) {
@@ -311,10 +318,9 @@ __device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const ui
             a0 = hfma2(wh[r][3], x0.w, a0); b0 = hfma2(wh[r][7], x1.w, b0);
             a1 = hfma2(wh[r][11], x2.w, a1); b1 = hfma2(wh[r][15], x3.w, b1);
             a0 = hadd2(a0, b0); a1 = hadd2(a1, b1);
-            const float2 f0 = h2_to_float2(a0), f1 = h2_to_float2(a1);
             const float p0 = sw[r][2 * j] * sx.x, p1 = sw[r][2 * j + 1] * sx.y;
-            acc[r][m] = fmaf(f0.x, p0, acc[r][m]); acc[r][m] = fmaf(f0.y, p0, acc[r][m]);
-            acc[r][m] = fmaf(f1.x, p1, acc[r][m]); acc[r][m] = fmaf(f1.y, p1, acc[r][m]);
+            acc[r][m] = fmaf(h2_sum_f32(a0), p0, acc[r][m]);    // f32(lo) + f32(hi): exact (|sum| <= 576)
+            acc[r][m] = fmaf(h2_sum_f32(a1), p1, acc[r][m]);
         }
     }
 }
