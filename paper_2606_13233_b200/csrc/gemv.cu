@@ -44,11 +44,10 @@ size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
 GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     GemvConfig c;
     const Layout L = make_layout(N, K, layout_kparts(N, K));
-    // from the round-1 sweeps on B200 (profiles/r01_sweep.md): two stages are enough once 16+ warps
-    // stream concurrently; R = 2 pays when the activation loads are not warp-uniform (KP > 1) or M is large
+    // from the round-1 sweeps on B200 (profiles/r01_sweep.md): with 4608-byte cells two stages per warp
+    // keep enough bytes in flight; one tile per warp (R = 1) and 12-16 consumer warps are best everywhere
     const bool half_path = (gemv_kmode(mode, M) == KMODE_W4A4_H);
     c.rows = 1;
-    if (mode == NVFP4_MODE_W4A4 && !half_path && (L.kp > 1 || M >= 8) && L.ntiles >= 4 * NUM_SMS) c.rows = 2;
     c.warps = (M >= 8 || half_path) ? 12 : 16;
     c.stages = 2;
     c.ksplit = 1;
