@@ -368,7 +368,7 @@ def run_ours(args):
 
 # per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from
 # the committed `ncu --set full` capture (profiles/); None until a capture exists for that M.
-TRAFFIC_BYTES_PER_STEP = {1: 279.55e6}    # profiles/r01_ncu_full_m1.md: 29.53 + 23.64 + 151.82 + 74.56 MB (algorithmic: 274.4 MB)
+TRAFFIC_BYTES_PER_STEP = {1: 279.19e6}    # profiles/r01_ncu_full_m1.md (algorithmic: 274.4 MB)
 
 
 def sweep(wl0, peak):
