@@ -106,6 +106,8 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     const int min_cells = (p.units / ctas) * (p.nch / cfg.ksplit);
     if (p.warps > min_cells) p.warps = min_cells;
     if (!(gemv_kmode(mode, M) == KMODE_W4A4_H && M == 1) && p.warps > 16) p.warps = 16;             // launch bounds: 1024 threads for M = 1, 640 otherwise
+    p.units_q = p.units / ctas; p.units_r = p.units % ctas;
+    p.cells_q = p.nch / cfg.ksplit; p.cells_r = p.nch % cfg.ksplit;
     dim3 grid(ctas, cfg.ksplit);
     const int threads = p.warps * 32 + STAGER_THREADS;
     const int kmode = gemv_kmode(mode, M);

@@ -40,6 +40,8 @@ struct GemvParams {
     int kp, kp_shift;              // K parts per row inside a warp (power of two) and its log2
     int warps, stages, ksplit;
     int units;                     // ceil(ntiles / R): work items shared by the gridDim.x CTAs of a K range
+    int units_q, units_r;          // units / gridDim.x and units % gridDim.x   (CTA bx gets q + (bx < r) units)
+    int cells_q, cells_r;          // nch / ksplit and nch % ksplit             (K range by gets q + (by < r) cells)
     int y_bf16;
     int zero;                      // always 0 (see make_wlut)
 };
@@ -509,15 +511,16 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
 
     // K range of this CTA (whole cells of 128*kp k)
-    const int c0 = (int)(((int64_t)blockIdx.y * p.nch) / p.ksplit);
-    const int c1 = (int)(((int64_t)(blockIdx.y + 1) * p.nch) / p.ksplit);
-    const int ncw = c1 - c0;
-    const int ncw_max = (p.nch + p.ksplit - 1) / p.ksplit;
+    // (quotients and remainders come from the host: no integer division in the prologue)
+    const int by = blockIdx.y, bx = blockIdx.x;
+    const int c0 = by * p.cells_q + (by < p.cells_r ? by : p.cells_r);
+    const int ncw = p.cells_q + (by < p.cells_r ? 1 : 0);
+    const int ncw_max = p.cells_q + (p.cells_r > 0 ? 1 : 0);
 
     // units of this CTA
-    const int u0 = (int)(((int64_t)blockIdx.x * p.units) / gridDim.x);
-    const int u1 = (int)(((int64_t)(blockIdx.x + 1) * p.units) / gridDim.x);
-    const int ucta_max = (p.units + gridDim.x - 1) / gridDim.x;
+    const int u0 = bx * p.units_q + (bx < p.units_r ? bx : p.units_r);
+    const int u1 = u0 + p.units_q + (bx < p.units_r ? 1 : 0);
+    const int ucta_max = p.units_q + (p.units_r > 0 ? 1 : 0);
     const int T = (u1 - u0) * ncw;                                          // cells of this CTA (>= W)
 
     // shared memory carve-up (must match gemv_smem_bytes)
@@ -551,6 +554,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     uint8_t* ring = ring_all + (size_t)warp * S * STAGE_BYTES;
     uint64_t* bars = bars_all + warp * S;
     const int f0 = fstart[warp], f1 = fstart[warp + 1];
+    const int f0_ul = (int)((unsigned)f0 / (unsigned)ncw);
     const int total = f1 - f0;
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
 
@@ -562,7 +566,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     const uint32_t ring_end = p_dst + (uint32_t)S * STAGE_BYTES;
     const uint8_t* p_src = nullptr;
     {
-        const int ul = f0 / ncw, cell = f0 - ul * ncw;
+        const int ul = f0_ul, cell = f0 - ul * ncw;
         const int tile0 = (u0 + ul) * R;
         p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
         p_left = ncw - cell;
@@ -607,7 +611,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
     const size_t xstep = (size_t)p.kp * XVS;
     const uint8_t* xlane0 = xs + (size_t)part * XVS;
-    int c_ul = f0 / ncw;
+    int c_ul = f0_ul;
     const int cell0 = f0 - c_ul * ncw;
     const uint8_t* xlane = xlane0 + (size_t)cell0 * CELL_VECS * xstep;
     // loop state kept incremental (no per-iteration index arithmetic): consumer stage pointer and
