@@ -48,7 +48,7 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K) {
     // keep enough bytes in flight; one tile per warp (R = 1) and 12-16 consumer warps are best everywhere
     const bool half_path = (gemv_kmode(mode, M) == KMODE_W4A4_H);
     c.rows = 1;
-    c.warps = (M >= 8 || half_path) ? 12 : 16;
+    c.warps = (M >= 8 || (half_path && K < 16384)) ? 12 : 16;
     c.stages = 2;
     c.ksplit = 1;
     // one persistent CTA per SM: shrink only if it does not fit in the 227 KB of shared memory

@@ -46,8 +46,9 @@ __host__ __device__ inline Layout make_layout(int N, int K, int kp) {
     return L;
 }
 
-// K parts for a weight shape: the smallest power of two that yields >= 1184 (= 148 SMs x 8 warps)
-// warp units, among those whose K padding costs at most 3% more than KP = 1 does.
+// K parts for a weight shape: the smallest power of two that yields >= 296 (= 2 per SM) tiles, among
+// those whose K padding costs at most 3% more than KP = 1 does.  (Balance inside an SM comes from the
+// in-CTA stream split, so few K parts are needed; fewer parts = more uniform activation loads.)
 __host__ __device__ inline int layout_kparts(int N, int K) {
 #ifndef __CUDA_ARCH__
     { const char* e = getenv("NVFP4_KP"); if (e) return atoi(e); }     // experiments only
@@ -60,7 +61,7 @@ __host__ __device__ inline int layout_kparts(int N, int K) {
         const long long padk = ((K + ck - 1) / ck) * ck;
         if (padk * 100 > pad1 * 103) break;
         best = kp;
-        if ((long long)N * kp >= 1184LL * 32) break;
+        if ((long long)N * kp >= 296LL * 32) break;
     }
     return best;
 }
