@@ -254,6 +254,23 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def max_over_ranks(ms, world, device):
+    """replicas-only multi-GPU contract: every rank runs the same step on its own GPU; the job's time is
+    the MAX over ranks (one all-reduce of a scalar; there is no data-path collective)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(bytes_per_rank_step, world, ms_step):
+    """whole-job throughput of `world` replicas (weak scaling): all ranks' bytes / the slowest rank's time."""
+    return world * bytes_per_rank_step / (ms_step * 1e-3) / 1e9
+
+
 # ---- our arm -----------------------------------------------------------------------------------
 def run_ours(args):
     import torch
@@ -286,10 +303,7 @@ def run_ours(args):
         ms_gemv = time_graph(torch, g_gemv, reps, wrep) / 2
         ms_q = time_graph(torch, g_q, reps, wrep) / 2
     barrier()
-    if world > 1:
-        t = torch.tensor([ms_step], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step = float(t.item())
+    ms_step = max_over_ranks(ms_step, world, "cuda")
 
     # end to end through the public API from pinned host buffers
     for c in range(max(3, args.warmup)):
@@ -302,14 +316,11 @@ def run_ours(args):
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1) / args.steps
-    if world > 1:
-        t = torch.tensor([ms_e2e], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, world, "cuda")
 
     b_step = wl.bytes_step(with_quant=True)
     b_gemv = wl.bytes_step(with_quant=False)
-    value = world * b_step / (ms_step * 1e-3) / 1e9
+    value = job_value(b_step, world, ms_step)
     ach = b_gemv / (ms_gemv * 1e-3) / 1e9
     h2d = sum(M * p["K"] * 2 for p in wl.proj)
     d2h = sum(M * p["N"] * 2 for p in wl.proj)
