@@ -2,7 +2,7 @@
 //   Y[m,n] = sum_k vX[m,k] * vW[n,k]     (CUDA cores only)
 //
 // Design (differs from the paper's FP16 cvt+hfma2 kernel):
-//  * lane <-> (weight row, K part): lane = r*KP + p.  A warp owns R tiles of 32/KP rows and walks
+//  * lane <-> (weight row, K part): lane = p*(32/KP) + r.  A warp owns R tiles of 32/KP rows and walks
 //    the CTA's K range; the KP lanes of a row take interleaved 32-k vectors and are summed by
 //    log2(KP) warp shuffles ONCE, after the K loop.  KP is a property of the repacked layout
 //    (nvfp4_common.cuh), chosen so that N*KP/32 independent warps fill the GPU: in the tuned
@@ -444,7 +444,7 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
                                                const int* fstart,
                                                int ul, int unit, bool whole, bool seg_at_share_start, int ncw, int T,
                                                int warp, int lane, int part, int rsub, int rpt, float gs) {
-    for (int off = 1; off < p.kp; off <<= 1) {
+    for (int off = rpt; off < 32; off <<= 1) {                  // lanes of one row are rpt apart
 #pragma unroll
         for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -505,7 +505,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
-    const int part = lane & (p.kp - 1), rsub = lane >> p.kp_shift;          // lane = rsub*kp + part
+    const int rsub = lane & ((32 >> p.kp_shift) - 1), part = lane >> (5 - p.kp_shift);   // lane = part*rpt + rsub
     const int rpt = 32 >> p.kp_shift;
     constexpr int XBP = xbp_bytes(MODE);
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;

@@ -17,7 +17,8 @@
 namespace nvfp4 {
 
 // ---- repacked weight blob geometry -------------------------
-// A lane of the GEMV owns (row r, K part p): lane = r*KP + p, KP = 2^i K parts per row inside a
+// A lane of the GEMV owns (row r, K part p): lane = p*(32/KP) + r (lanes of one K part are adjacent,
+// so their activation loads hit one address per part), KP = 2^i K parts per row inside a
 // warp (chosen per weight shape by layout_kparts, so that N*KP/32 independent warp units fill
 // the 148 SMs without any cross-warp or cross-CTA reduction).  A "cell" is what one warp consumes
 // in CELL_VECS = 8 128-bit loads per lane: 32/KP weight rows x 256*KP consecutive k:
@@ -46,8 +47,8 @@ __host__ __device__ inline Layout make_layout(int N, int K, int kp) {
     return L;
 }
 
-// K parts for a weight shape: the smallest power of two that yields >= 296 (= 2 per SM) tiles, among
-// those whose K padding costs at most 3% more than KP = 1 does.  (Balance inside an SM comes from the
+// K parts for a weight shape: the smallest power of two that yields >= 296 (= 2 per SM) tiles of at most
+// 32 cells each, among those whose K padding costs at most 3% more than KP = 1 does.  (Balance inside an SM comes from the
 // in-CTA stream split, so few K parts are needed; fewer parts = more uniform activation loads.)
 __host__ __device__ inline int layout_kparts(int N, int K) {
 #ifndef __CUDA_ARCH__
@@ -61,7 +62,8 @@ __host__ __device__ inline int layout_kparts(int N, int K) {
         const long long padk = ((K + ck - 1) / ck) * ck;
         if (padk * 100 > pad1 * 103) break;
         best = kp;
-        if ((long long)N * kp >= 296LL * 32) break;
+        // enough tiles (2 per SM), and rows short enough (<= 32 cells) that a row tile is shared by few warps
+        if ((long long)N * kp >= 296LL * 32 && padk / ck <= 32) break;
     }
     return best;
 }

@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes
         const int tile = (int)(cell / L.ncells), ci = (int)(cell - (int64_t)tile * L.ncells);
         uint8_t* cellp = blob + cell * CELL_BYTES;
         const int lane = e & 31;
-        const int n = tile * L.rpt + lane / L.kp, part = lane % L.kp;
+        const int n = tile * L.rpt + lane % L.rpt, part = lane / L.rpt;      // lane = part * rpt + row
         if (e < CELL_VECS * 32) {
             const int j = e >> 5;
             const int64_t k0 = (int64_t)ci * L.cell_k + (int64_t)(j * L.kp + part) * 32;
