@@ -178,8 +178,8 @@ static cudaError_t launch_cluster(int nctas, int threads, cudaStream_t st, const
     attr[0].val.clusterDim.x = nctas;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 2;
+    if (nctas > 1) { cfg.attrs = attr; cfg.numAttrs = 2; }
+    else           { cfg.attrs = attr + 1; cfg.numAttrs = 1; }      // single CTA: no cluster launch needed
     return cudaLaunchKernelEx(&cfg, quantize_act_kernel<BPT, DYN>, x, M, K, ldx, codes, scales, gscale);
 }
 
