@@ -128,6 +128,22 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
                void* workspace, size_t ws_bytes, void* stream);
 
 /*
+ * Fused variant of the two calls above: W4A4 GEMV on BF16 activations with the
+ * activation quantizer (dynamic global scale, same bit-exact op sequence as nvfp4_quantize_act) run inside
+ * the GEMV kernel -- one launch instead of two.  The result equals nvfp4_quantize_act followed by
+ * nvfp4_gemv(NVFP4_MODE_W4A4) on the same inputs (bit-identical at M = 1, where both use the same
+ * arithmetic path; within the tolerance for M >= 2).  Every CTA re-quantises the activations it needs, so
+ * this pays for small M (<= 2); the canonical codes / scales are not materialised.
+ *   x_bf16        [device] BF16 bits, row m at x_bf16 + m*ldx elements; ldx >= K, ldx % 8 == 0
+ *   x_gscale_out  [device] optional (may be NULL): receives the activation global scale amax/2688
+ * Other arguments as for nvfp4_gemv; workspace as returned by nvfp4_gemv_workspace_bytes.
+ */
+int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int K,
+                           const void* x_bf16, int M, int64_t ldx, float* x_gscale_out,
+                           void* y, int y_dtype, int64_t ldy,
+                           void* workspace, size_t ws_bytes, void* stream);
+
+/*
  * Launch-shape override for sweeps (host-side state, not thread-safe; 0 = use the tuned table):
  *   ksplit = number of K ranges (grid.y, 1..64), warps = warps per CTA (1..16),
  *   rows   = 32-row weight tiles per warp, i.e. weight rows per lane (1, 2 or 4),

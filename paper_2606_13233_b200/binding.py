@@ -24,7 +24,7 @@ ERR_NAMES = {0: "NVFP4_OK", -1: "NVFP4_ERR_INVALID_ARG", -2: "NVFP4_ERR_UNSUPPOR
 # every symbol include/nvfp4.h declares (tests check that the library exports all of them)
 SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp4_repacked_bytes",
            "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
-           "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul")
+           "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant")
 
 
 class Nvfp4Error(RuntimeError):
@@ -56,6 +56,8 @@ def _load():
     lib.nvfp4_gemv.restype = c_int
     lib.nvfp4_gemv.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64,
                                vp, c_sz, vp]
+    lib.nvfp4_gemv_fused_quant.restype = c_int
+    lib.nvfp4_gemv_fused_quant.argtypes = [vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_set_config.restype = c_int
     lib.nvfp4_gemv_set_config.argtypes = [c_int, c_int, c_int, c_int]
     lib.nvfp4_gemv_get_config.restype = c_int
@@ -138,6 +140,20 @@ def nvfp4_gemv(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, y=
         workspace = new_workspace(M, N, K, x.device)
     _check(lib.nvfp4_gemv(mode, _ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x), _ptr(x_scales), _ptr(x_gscale), M,
                           x.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
+    return y
+
+
+def nvfp4_gemv_fused_quant(w_blob, w_gscale, N, K, x_bf16, x_gscale_out=None, y=None, y_dtype=DTYPE_BF16,
+                           workspace=None):
+    """quantize_act + W4A4 gemv in ONE launch; x_bf16 [M,K] torch.bfloat16.  Returns y [M,N]."""
+    M = x_bf16.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x_bf16.device)
+    if workspace is None:
+        workspace = new_workspace(M, N, K, x_bf16.device)
+    _check(lib.nvfp4_gemv_fused_quant(_ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x_bf16), M, x_bf16.stride(0),
+                                      _ptr(x_gscale_out), _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
+                                      workspace.numel(), _stream()))
     return y
 
 

@@ -79,7 +79,8 @@ size_t nvfp4_gemv_workspace_bytes(int M, int N, int K) {
     if (!shape_ok(M, N, K)) return 0;
     const size_t a = gemv_workspace_bytes_for(M, N, K, effective_config(NVFP4_MODE_W4A4, M, N, K));
     const size_t b = gemv_workspace_bytes_for(M, N, K, effective_config(NVFP4_MODE_W4A16, M, N, K));
-    return a > b ? a : b;
+    const size_t c = gemv_workspace_bytes_for(M, N, K, effective_config(MODE_W4A4_FUSED_QUANT, M, N, K));
+    return a > b ? (a > c ? a : c) : (b > c ? b : c);
 }
 
 int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K, const void* x,
@@ -100,6 +101,23 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
     if (cfg.ksplit > 1 && (!workspace || ws_bytes < need)) return NVFP4_ERR_INVALID_ARG;
     cudaError_t e = launch_gemv(mode, w_blob, w_gscale, N, K, x, x_scales, x_gscale, M, ldx, y, y_dtype, ldy,
                                 workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int K, const void* x_bf16, int M,
+                           int64_t ldx, float* x_gscale_out, void* y, int y_dtype, int64_t ldy,
+                           void* workspace, size_t ws_bytes, void* stream) {
+    g_last_err[0] = 0;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob || !w_gscale || !x_bf16 || !y) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(M, N, K) || ldy < N || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob) || !aligned16(x_bf16) || !aligned16(y) || (workspace && !aligned16(workspace)))
+        return NVFP4_ERR_ALIGNMENT;
+    const GemvConfig cfg = effective_config(MODE_W4A4_FUSED_QUANT, M, N, K);
+    const size_t need = gemv_workspace_bytes_for(M, N, K, cfg);
+    if (cfg.ksplit > 1 && (!workspace || ws_bytes < need)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemv(MODE_W4A4_FUSED_QUANT, w_blob, w_gscale, N, K, x_bf16, nullptr, x_gscale_out, M, ldx,
+                                y, y_dtype, ldy, workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 

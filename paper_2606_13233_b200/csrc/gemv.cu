@@ -12,6 +12,7 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // arithmetic variant: W4A4 runs the FP16 path up to M = NVFP4_MH (default 1), the integer path above
 int gemv_kmode(int mode, int M) {
     if (mode == NVFP4_MODE_W4A16) return KMODE_W4A16;
+    if (mode == MODE_W4A4_FUSED_QUANT) return KMODE_W4A4_H;     // the fused stagers write f16 records
     static int mh = -1;
     if (mh < 0) { const char* e = getenv("NVFP4_MH"); mh = e ? atoi(e) : 1; }
     return M <= mh ? KMODE_W4A4_H : KMODE_W4A4_I8;
@@ -36,7 +37,7 @@ size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
          + (size_t)c.warps * 2 * c.rows * M * L.rpt * sizeof(float)          // segment slots
          + (size_t)c.warps * c.stages * 8                                    // ring mbarriers
          + ((size_t)ncw_max * L.kp * M * 4 * CELL_VECS / STAGE_ITEMS + 2) * 8          // staging-batch mbarriers
-         + (size_t)(ucta_max + c.warps + 4) * sizeof(int);                   // unit counters + share starts
+         + (size_t)(ucta_max + c.warps + 16) * sizeof(int);                  // unit counters + share starts + fused-quant scratch
 }
 
 // Launch shape per (mode, M, N, K).  Values come from the sweeps recorded in DESIGN.md
@@ -81,6 +82,7 @@ cudaError_t launch_gemv_w4a4h(const GemvParams& p, int M, int R, dim3 grid, int 
 cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, const void* x,
                         const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
                         int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st) {
+    const bool fuse_quant = (mode == MODE_W4A4_FUSED_QUANT);
     GemvParams p;
     p.blob = static_cast<const uint8_t*>(blob);
     p.w_gscale = w_gscale;
@@ -97,6 +99,8 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     p.warps = cfg.warps; p.stages = cfg.stages; p.ksplit = cfg.ksplit;
     p.y_bf16 = (y_dtype == NVFP4_DTYPE_BF16);
     p.zero = 0;
+    p.fuse_quant = fuse_quant ? 1 : 0;
+    p.x_gscale_out = fuse_quant ? const_cast<float*>(x_gscale) : nullptr;
     if (cfg.ksplit > 1 && ws_bytes < gemv_workspace_bytes_for(M, N, K, cfg)) return cudaErrorInvalidValue;
     const size_t smem = gemv_smem_bytes(mode, M, N, K, cfg);
     if (smem > SMEM_CAP) return cudaErrorInvalidConfiguration;

@@ -6,6 +6,10 @@
 
 namespace nvfp4 {
 
+// internal `mode` value (beyond NVFP4_MODE_W4A4 / _W4A16): W4A4 with the activation quantizer fused into
+// the GEMV's stagers -- x is BF16, x_scales is NULL, x_gscale is an optional OUTPUT
+constexpr int MODE_W4A4_FUSED_QUANT = 2;
+
 // launch shape of the GEMV: every field > 0
 struct GemvConfig {
     int warps;    // warps per CTA, each owns `rows` row tiles (32 rows each) -> no cross-warp reduce

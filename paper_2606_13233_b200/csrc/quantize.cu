@@ -9,6 +9,7 @@
 
 #include "nvfp4_common.cuh"
 #include "nvfp4_internal.h"
+#include "quant_block.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -17,29 +18,14 @@ namespace nvfp4 {
 constexpr int QTHREADS_MAX = 1024;
 constexpr int QCLUSTER_MAX = 8;
 
-__device__ __forceinline__ uint32_t absmax_bits16(const uint4& a, const uint4& b) {
-    // max over the sixteen 15-bit magnitudes (BF16 magnitudes order like integers)
-    uint32_t m = 0;
-    const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        uint32_t v = w[i] & 0x7FFF7FFFu;
-        m = max(m, max(v & 0xFFFFu, v >> 16));
-    }
-    return m;
-}
-
 // quantise one 16-element block held as 8 packed BF16 pairs; returns 8 code bytes + scale byte
 __device__ __forceinline__ void quantize_block(const uint4& a, const uint4& b, uint32_t ab_bits, float g,
                                                uint2& out_codes, uint8_t& out_scale) {
     out_codes = make_uint2(0u, 0u);
     out_scale = 0;
     if (!(g > 0.0f)) return;                                   // amax == 0 (or bad static g): all zero
-    const float a_b = __uint_as_float(ab_bits << 16);
-    const float t = __fdiv_rn(a_b, 6.0f);
-    const float u = __fdiv_rn(t, g);
-    const uint8_t sc = float_to_e4m3_rn_sat(fminf(u, 448.0f));
-    const float d = __fmul_rn(g, e4m3_to_float(sc));
+    uint8_t sc; float d;
+    block_scale(ab_bits, g, sc, d);
     out_scale = sc;
     if (d == 0.0f) return;                                     // flushed block (R5): codes 0x0
     const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
