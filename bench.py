@@ -129,6 +129,22 @@ class Workload:
                 gx=torch.zeros(1, dtype=torch.float32, device="cuda"),
                 y=torch.empty((M, N), dtype=torch.bfloat16, device="cuda"),
                 ws=B.new_workspace(M, N, K)))
+        # e2e staging: the step's four activations / outputs as ONE pinned host buffer and ONE device buffer each
+        # (element offsets are multiples of 8 BF16 = 16 B), so a step costs one H2D and one D2H copy
+        def pack(key, host_key):
+            n = sum(p[key].numel() for p in self.proj)
+            dev = torch.empty(n, dtype=torch.bfloat16, device="cuda")
+            host = torch.empty(n, dtype=torch.bfloat16).pin_memory()
+            off = 0
+            for p in self.proj:
+                k = p[key].numel()
+                dev[off:off + k].copy_(p[key].reshape(-1))
+                host[off:off + k].copy_(p[host_key].reshape(-1))
+                p[key] = dev[off:off + k].view(p[key].shape)
+                off += k
+            return dev, host
+        self.x_all, self.x_all_host = pack("x", "x_host")
+        self.y_all, self.y_all_host = pack("y", "y_host")
         torch.cuda.synchronize()
 
     # -- one projection, all on the current stream ------------------------------------------
@@ -144,10 +160,15 @@ class Workload:
             B.nvfp4_gemv(B.MODE_W4A16, p["blobs"][copy], p["gw"], p["N"], p["K"], p["x"],
                          y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
 
-    def step(self, copy, quant=True, gemv=True, only=None):
+    def step(self, copy, quant=True, gemv=True, only=None, fused=False):
         n = 0
         for p in self.proj:
             if only is not None and p["name"] != only:
+                continue
+            if fused:          # one launch: quantizer inside the GEMV (nvfp4_gemv_fused_quant)
+                self.B.nvfp4_gemv_fused_quant(p["blobs"][copy], p["gw"], p["N"], p["K"], p["x"], p["gx"], y=p["y"],
+                                              y_dtype=self.B.DTYPE_BF16, workspace=p["ws"])
+                n += 1
                 continue
             if quant and self.mode == "w4a4":
                 self.quantize(p); n += 1
@@ -174,12 +195,12 @@ class Workload:
 
     def step_e2e(self, copy):
         """public-API path from HOST buffers: H2D activations, quantize, gemv, D2H outputs."""
+        self.x_all.copy_(self.x_all_host, non_blocking=True)          # H2D: the step's BF16 activations
         for p in self.proj:
-            p["x"].copy_(p["x_host"], non_blocking=True)
             if self.mode == "w4a4":
                 self.quantize(p)
             self.gemv(p, copy)
-            p["y_host"].copy_(p["y"], non_blocking=True)
+        self.y_all_host.copy_(self.y_all, non_blocking=True)          # D2H: the step's BF16 outputs
 
     def bytes_step(self, with_quant=True):
         return sum(algorithmic_bytes(self.M, p["N"], p["K"], with_quant) for p in self.proj)
@@ -288,6 +309,7 @@ def run_ours(args):
     g_step, n_step = wl.capture(2)
     g_gemv, n_gemv = wl.capture(2, quant=False)
     g_q, n_q = wl.capture(2, gemv=False)
+    g_fused, n_fused = wl.capture(2, fused=True)
     reps = max(1, (args.steps + 1) // 2)            # one replay = 2 steps
     wrep = max(2, (args.warmup + 1) // 2)
 
@@ -302,6 +324,7 @@ def run_ours(args):
         # keep the sampler running over the kernel-only graphs too (same clocks regime)
         ms_gemv = time_graph(torch, g_gemv, reps, wrep) / 2
         ms_q = time_graph(torch, g_q, reps, wrep) / 2
+        ms_fused = time_graph(torch, g_fused, reps, wrep) / 2
     barrier()
     ms_step = max_over_ranks(ms_step, world, "cuda")
 
@@ -371,6 +394,8 @@ def run_ours(args):
                        "multi_gpu": "replicas only"},
             "us_per_projection": {"step_mean": round(ms_step * 1e3 / 4, 2), "gemv_mean": round(ms_gemv * 1e3 / 4, 2),
                                   "quantize_mean": round(ms_q * 1e3 / 4, 2), "per_shape_gemv": per_shape},
+            "fused_step": {"what": "same step with nvfp4_gemv_fused_quant (quantizer inside the GEMV: 4 launches)",
+                           "ms_per_step": ms_fused, "value": job_value(b_step, world, ms_fused), "unit": UNIT},
             "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone)",
                          "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": ach / peak,
                          "traffic": TRAFFIC_BYTES_PER_STEP.get(M)},
@@ -468,8 +493,8 @@ def run_chain(args):
     import torch
     from paper_2606_13233_b200.chain import DecodeChain
     peak, _ = measured_peak()
-    for M in (1, 2, 4, 8):
-        ch = DecodeChain(layers=args.layers, M=M)
+    for M, fused in ((1, False), (2, False), (4, False), (8, False), (1, True), (2, True)):
+        ch = DecodeChain(layers=args.layers, M=M, fused=fused)
         h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
         ch.calibrate(h0)
         ch.step()
@@ -481,7 +506,7 @@ def run_chain(args):
         ms = time_graph(torch, g, 20, 3)
         finite = bool(torch.isfinite(ch.h.float()).all())
         wb = ch.weight_bytes()
-        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "ms_per_token": round(ms, 4),
+        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "fused_quant": fused, "ms_per_token": round(ms, 4),
                           "us_per_layer": round(ms * 1e3 / args.layers, 2), "weight_gb": round(wb / 1e9, 2),
                           "gbs": round(wb / ms / 1e6, 1), "frac_of_copy_peak": round(wb / ms / 1e6 / peak, 3),
                           "launches": ch.launches_per_step, "finite": finite}), flush=True)

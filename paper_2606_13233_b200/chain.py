@@ -19,7 +19,8 @@ QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
 
 
 class DecodeChain:
-    def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda"):
+    def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False):
+        self.fused = fused                            # one nvfp4_gemv_fused_quant launch per projection
         d = dict(QWEN3_32B_DIMS if dims is None else dims)
         self.M, self.layers, self.d = M, layers, d
         H, QKV, OIN, I = d["hidden"], d["qkv"], d["o_in"], d["inter"]
@@ -47,13 +48,16 @@ class DecodeChain:
         self.xs = torch.empty((M, kmax // 16), dtype=u8, device=device)
         self.gx = torch.zeros(1, dtype=torch.float32, device=device)
         self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
-        self.launches_per_step = layers * 9
+        self.launches_per_step = layers * (5 if fused else 9)
 
     def set_input(self, h_bf16):
         self.h.copy_(h_bf16)
 
     def _proj(self, l, i, x, y):
         blob, gw, N, K = self.w[l][i]
+        if self.fused:
+            B.nvfp4_gemv_fused_quant(blob, gw, N, K, x, self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])
+            return
         xc = self.xc.view(-1)[: self.M * (K // 2)].view(self.M, K // 2)
         xs = self.xs.view(-1)[: self.M * (K // 16)].view(self.M, K // 16)
         B.nvfp4_quantize_act(x, xc, xs, self.gx)
