@@ -36,8 +36,8 @@ size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c) {
     return xs + (size_t)c.warps * c.stages * c.rows * CELL_BYTES             // rings
          + (size_t)c.warps * 2 * c.rows * M * L.rpt * sizeof(float)          // segment slots
          + (size_t)c.warps * c.stages * 8                                    // ring mbarriers
-         + ((size_t)ncw_max * L.kp * M * 4 * CELL_VECS / STAGE_ITEMS + 2) * 8          // staging-batch mbarriers
-         + (size_t)(ucta_max + c.warps + 16) * sizeof(int);                  // unit counters + share starts + fused-quant scratch
+         + ((size_t)ncw_max * L.kp * M * 4 * CELL_VECS / (mode == MODE_W4A4_FUSED_QUANT ? 160 : STAGE_ITEMS) + 2) * 8   // staging-batch mbarriers
+         + (size_t)(ucta_max + c.warps + 40) * sizeof(int);                  // unit counters + share starts + fused-quant scratch
 }
 
 // Launch shape per (mode, M, N, K).  Values come from the sweeps recorded in DESIGN.md

@@ -190,28 +190,28 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
     }
 }
 
-// Fused quantization (nvfp4_gemv_fused_quant): the stagers run the activation quantizer themselves --
+// Fused quantization (nvfp4_gemv_fused_quant): ALL threads of the CTA run the activation quantizer themselves --
 // pass 1: tensor-wide amax of the BF16 activations (whole [M,K], every CTA redundantly: <= 410 KB from L2),
 // pass 2: per 16-block the R2 sequence of quant_block.cuh, then straight to the f16 record (the E2M1 code is
 // produced by cvt.rn.satfinite.e2m1x2.f32 and expanded by cvt.rn.f16x2.e2m1x2, so the values are exactly
 // those of quantize_act followed by the normal staging).  `red` = 8 words of shared memory.
 template <int M>
-__device__ __forceinline__ void stage_x_fused_h(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
+__device__ __forceinline__ void stage_x_fused_h(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
                                                 uint64_t* xbars, uint32_t* red, float* gx_slot) {
+    // called by EVERY thread of the CTA (consumer warps right after they have started their weight stream)
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
     const int kb_total = p.K >> 4;
     uint32_t tmax = 0;
-    for (int i = tid; i < kb_total * M; i += STAGER_THREADS) {
+    for (int i = tid; i < kb_total * M; i += nthr) {
         const int m = i / kb_total, kb = i - m * kb_total;
         const uint4* src = reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + (int64_t)kb * 16);
         tmax = max(tmax, absmax_bits16(__ldg(src), __ldg(src + 1)));
     }
     tmax = __reduce_max_sync(0xFFFFFFFFu, tmax);
     if ((tid & 31) == 0) red[tid >> 5] = tmax;
-    asm volatile("bar.sync 1, %0;" ::"n"(STAGER_THREADS) : "memory");
+    asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory");
     uint32_t amax_bits = 0;
-#pragma unroll
-    for (int w = 0; w < STAGER_WARPS; ++w) amax_bits = max(amax_bits, red[w]);
+    for (int w = 0; w < (nthr >> 5); ++w) amax_bits = max(amax_bits, red[w]);
     const float g = __fdiv_rn(__uint_as_float(amax_bits << 16), 2688.0f);
     if (tid == 0) {
         *gx_slot = g;
@@ -220,37 +220,34 @@ __device__ __forceinline__ void stage_x_fused_h(const GemvParams& p, uint8_t* xs
     const int nblk = ncw * 2 * CELL_VECS * p.kp;
     const int kb0 = c0 * 2 * CELL_VECS * p.kp;
     const int total = nblk * M;
-    for (int base = 0; base < total; base += STAGE_ITEMS) {
-#pragma unroll 2
-        for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = base + t * STAGER_THREADS + tid;
-            if (i < total) {
-                const int blk = i / M, m = i - blk * M;
-                uint8_t* rec = xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_H, M) + m * XBP_W4A4H;
-                uint32_t h[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
-                float sx = 0.0f;
-                if (kb0 + blk < kb_total && g > 0.0f) {
-                    const uint4* src = reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + (int64_t)(kb0 + blk) * 16);
-                    const uint4 a = __ldg(src), b = __ldg(src + 1);
-                    uint8_t sc; float d;
-                    block_scale(absmax_bits16(a, b), g, sc, d);
-                    sx = e4m3_to_float(sc);
-                    if (d != 0.0f) {
-                        const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+    for (int base = 0, batch = 0; base < total; base += nthr, ++batch) {     // one block per thread and batch
+        const int i = base + tid;
+        if (i < total) {
+            const int blk = i / M, m = i - blk * M;
+            uint8_t* rec = xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_H, M) + m * XBP_W4A4H;
+            uint32_t h[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+            float sx = 0.0f;
+            if (kb0 + blk < kb_total && g > 0.0f) {
+                const uint4* src = reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + (int64_t)(kb0 + blk) * 16);
+                const uint4 a = __ldg(src), b = __ldg(src + 1);
+                uint8_t sc; float d;
+                block_scale(absmax_bits16(a, b), g, sc, d);
+                sx = e4m3_to_float(sc);
+                if (d != 0.0f) {
+                    const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            const float x0 = __uint_as_float(w[e] << 16), x1 = __uint_as_float(w[e] & 0xFFFF0000u);
-                            h[e] = e2m1x2_to_f16x2(float2_to_e2m1x2(__fdiv_rn(x0, d), __fdiv_rn(x1, d)));
-                        }
+                    for (int e = 0; e < 8; ++e) {
+                        const float x0 = __uint_as_float(w[e] << 16), x1 = __uint_as_float(w[e] & 0xFFFF0000u);
+                        h[e] = e2m1x2_to_f16x2(float2_to_e2m1x2(__fdiv_rn(x0, d), __fdiv_rn(x1, d)));
                     }
                 }
-                uint4* dst = reinterpret_cast<uint4*>(rec + (blk & 1) * 32);
-                dst[0] = make_uint4(h[0], h[1], h[2], h[3]);
-                dst[1] = make_uint4(h[4], h[5], h[6], h[7]);
-                *reinterpret_cast<float*>(rec + 64 + (blk & 1) * 4) = sx;
             }
+            uint4* dst = reinterpret_cast<uint4*>(rec + (blk & 1) * 32);
+            dst[0] = make_uint4(h[0], h[1], h[2], h[3]);
+            dst[1] = make_uint4(h[4], h[5], h[6], h[7]);
+            *reinterpret_cast<float*>(rec + 64 + (blk & 1) * 4) = sx;
         }
-        mbar_arrive(smem_u32(xbars + base / STAGE_ITEMS));
+        mbar_arrive(smem_u32(xbars + batch));
     }
 }
 
@@ -598,14 +595,17 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     float* slots = reinterpret_cast<float*>(ring_all + (size_t)W * S * STAGE_BYTES);
     uint64_t* bars_all = reinterpret_cast<uint64_t*>(slots + (size_t)W * 2 * R * M * rpt);
     const int xitems = ncw_max * p.kp * M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2);  // staging items (upper bound)
-    const int nxb = (xitems + STAGE_ITEMS - 1) / STAGE_ITEMS;
+    const bool fused = (MODE == KMODE_W4A4_H) && p.fuse_quant;
+    const int stage_items = fused ? (int)blockDim.x : STAGE_ITEMS;          // items per staging batch
+    const int nxb = (xitems + stage_items - 1) / stage_items;
     uint64_t* xbars = bars_all + W * S;
     int* cnt = reinterpret_cast<int*>(xbars + nxb);
     int* fstart = cnt + ucta_max;
 
     for (int i = threadIdx.x; i < ucta_max; i += blockDim.x) cnt[i] = 0;
     if (threadIdx.x <= W) fstart[threadIdx.x] = flat_start(threadIdx.x, T, W);
-    if (threadIdx.x < nxb) mbar_init(smem_u32(xbars + threadIdx.x), STAGER_THREADS);
+    for (int i = threadIdx.x; i < nxb; i += blockDim.x)
+        mbar_init(smem_u32(xbars + i), fused ? blockDim.x : STAGER_THREADS);
     if (threadIdx.x == 0) mbar_fence_init();
     __syncthreads();
 
@@ -614,8 +614,8 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
         pdl_wait();                                   // the activations come from the previous kernel
         if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, tid, xbars);
         else if (MODE == KMODE_W4A4_H && p.fuse_quant)
-            stage_x_fused_h<M>(p, xs, c0, ncw, tid, xbars, reinterpret_cast<uint32_t*>(fstart + W + 4),
-                               reinterpret_cast<float*>(fstart + W + 2));
+            stage_x_fused_h<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
+                               reinterpret_cast<uint32_t*>(fstart + W + 4), reinterpret_cast<float*>(fstart + W + 2));
         else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, tid, xbars);
         return;
     }
@@ -669,7 +669,9 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     pdl_launch_dependents();
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
-    const bool fused = (MODE == KMODE_W4A4_H) && p.fuse_quant;
+    if (fused)      // consumers take their share of the quantization while their first weight cells are in flight
+        stage_x_fused_h<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
+                           reinterpret_cast<uint32_t*>(fstart + W + 4), reinterpret_cast<float*>(fstart + W + 2));
     const float gx_raw = (MODE == KMODE_W4A16 || fused) ? 1.0f : __ldg(p.x_gscale);
 
     float acc[R][M];
@@ -700,7 +702,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     uint32_t xbar = smem_u32(xbars);
     __syncwarp();
     for (int f = 0; f < total; ++f) {
-        while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += STAGE_ITEMS; }
+        while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += stage_items; }
         mbar_wait(bar, phase);
 
 #pragma unroll

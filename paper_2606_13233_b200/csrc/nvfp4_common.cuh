@@ -52,7 +52,10 @@ __host__ __device__ inline Layout make_layout(int N, int K, int kp) {
 // in-CTA stream split, so few K parts are needed; fewer parts = more uniform activation loads.)
 __host__ __device__ inline int layout_kparts(int N, int K) {
 #ifndef __CUDA_ARCH__
-    { const char* e = getenv("NVFP4_KP"); if (e) return atoi(e); }     // experiments only
+    {   // experiments only (read once): NVFP4_KP forces the K-part count of the layout
+        static const int forced = [] { const char* e = getenv("NVFP4_KP"); return e ? atoi(e) : 0; }();
+        if (forced > 0) return forced;
+    }
 #endif
     const long long ck1 = 32 * CELL_VECS;
     const long long pad1 = ((K + ck1 - 1) / ck1) * ck1;
