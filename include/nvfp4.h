@@ -131,9 +131,9 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
  * Fused variant of the two calls above: W4A4 GEMV on BF16 activations with the
  * activation quantizer (dynamic global scale, same bit-exact op sequence as nvfp4_quantize_act) run inside
  * the GEMV kernel -- one launch instead of two.  The result equals nvfp4_quantize_act followed by
- * nvfp4_gemv(NVFP4_MODE_W4A4) on the same inputs (bit-identical at M = 1, where both use the same
- * arithmetic path; within the tolerance for M >= 2).  Every CTA re-quantises the activations it needs, so
- * this pays for small M (<= 2); the canonical codes / scales are not materialised.
+ * nvfp4_gemv(NVFP4_MODE_W4A4) on the same inputs (same arithmetic path per M; bit-identical outputs are
+ * tested at M = 1).  Every CTA re-quantises the activations it needs, so this pays only at M = 1 (measured:
+ * DESIGN.md 6.4); the canonical codes / scales are not materialised.
  *   x_bf16        [device] BF16 bits, row m at x_bf16 + m*ldx elements; ldx >= K, ldx % 8 == 0
  *   x_gscale_out  [device] optional (may be NULL): receives the activation global scale amax/2688
  * Other arguments as for nvfp4_gemv; workspace as returned by nvfp4_gemv_workspace_bytes.

@@ -12,7 +12,6 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // arithmetic variant: W4A4 runs the FP16 path up to M = NVFP4_MH (default 1), the integer path above
 int gemv_kmode(int mode, int M) {
     if (mode == NVFP4_MODE_W4A16) return KMODE_W4A16;
-    if (mode == MODE_W4A4_FUSED_QUANT) return KMODE_W4A4_H;     // the fused stagers write f16 records
     static int mh = -1;
     if (mh < 0) { const char* e = getenv("NVFP4_MH"); mh = e ? atoi(e) : 1; }
     return M <= mh ? KMODE_W4A4_H : KMODE_W4A4_I8;

@@ -45,7 +45,7 @@ struct GemvParams {
     int cells_q, cells_r;          // nch / ksplit and nch % ksplit             (K range by gets q + (by < r) cells)
     int y_bf16;
     int zero;                      // always 0 (see make_wlut)
-    int fuse_quant;                // x is BF16 [M,K] (ldx elements): quantise it in the stagers (KMODE_W4A4_H only)
+    int fuse_quant;                // x is BF16 [M,K] (ldx elements): quantise it inside the kernel (W4A4 modes)
     float* x_gscale_out;           // fuse_quant: optional device float that receives the activation global scale
 };
 
@@ -195,8 +195,8 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
 // pass 2: per 16-block the R2 sequence of quant_block.cuh, then straight to the f16 record (the E2M1 code is
 // produced by cvt.rn.satfinite.e2m1x2.f32 and expanded by cvt.rn.f16x2.e2m1x2, so the values are exactly
 // those of quantize_act followed by the normal staging).  `red` = 8 words of shared memory.
-template <int M>
-__device__ __forceinline__ void stage_x_fused_h(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
+template <int M, bool HALF>
+__device__ __forceinline__ void stage_x_fused(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
                                                 uint64_t* xbars, uint32_t* red, float* gx_slot) {
     // called by EVERY thread of the CTA (consumer warps right after they have started their weight stream)
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
@@ -224,8 +224,9 @@ __device__ __forceinline__ void stage_x_fused_h(const GemvParams& p, uint8_t* xs
         const int i = base + tid;
         if (i < total) {
             const int blk = i / M, m = i - blk * M;
-            uint8_t* rec = xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_H, M) + m * XBP_W4A4H;
-            uint32_t h[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+            constexpr int KM = HALF ? KMODE_W4A4_H : KMODE_W4A4_I8;
+            uint8_t* rec = xs + (size_t)(blk >> 1) * xvec_stride(KM, M) + m * xbp_bytes(KM);
+            uint32_t h[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};        // HALF: f16 pairs; else: one code byte each
             float sx = 0.0f;
             if (kb0 + blk < kb_total && g > 0.0f) {
                 const uint4* src = reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + (int64_t)(kb0 + blk) * 16);
@@ -238,14 +239,21 @@ __device__ __forceinline__ void stage_x_fused_h(const GemvParams& p, uint8_t* xs
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const float x0 = __uint_as_float(w[e] << 16), x1 = __uint_as_float(w[e] & 0xFFFF0000u);
-                        h[e] = e2m1x2_to_f16x2(float2_to_e2m1x2(__fdiv_rn(x0, d), __fdiv_rn(x1, d)));
+                        const uint32_t byte = float2_to_e2m1x2(__fdiv_rn(x0, d), __fdiv_rn(x1, d));
+                        h[e] = HALF ? e2m1x2_to_f16x2(byte) : byte;
                     }
                 }
             }
-            uint4* dst = reinterpret_cast<uint4*>(rec + (blk & 1) * 32);
-            dst[0] = make_uint4(h[0], h[1], h[2], h[3]);
-            dst[1] = make_uint4(h[4], h[5], h[6], h[7]);
-            *reinterpret_cast<float*>(rec + 64 + (blk & 1) * 4) = sx;
+            if (HALF) {
+                uint4* dst = reinterpret_cast<uint4*>(rec + (blk & 1) * 32);
+                dst[0] = make_uint4(h[0], h[1], h[2], h[3]);
+                dst[1] = make_uint4(h[4], h[5], h[6], h[7]);
+                *reinterpret_cast<float*>(rec + 64 + (blk & 1) * 4) = sx;
+            } else {        // canonical code bytes -> the integer record (same routine as the normal staging)
+                const uint2 cw = make_uint2(h[0] | (h[1] << 8) | (h[2] << 16) | (h[3] << 24),
+                                            h[4] | (h[5] << 8) | (h[6] << 16) | (h[7] << 24));
+                decode_x_block(cw, sx, rec, blk & 1);
+            }
         }
         mbar_arrive(smem_u32(xbars + batch));
     }
@@ -595,7 +603,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     float* slots = reinterpret_cast<float*>(ring_all + (size_t)W * S * STAGE_BYTES);
     uint64_t* bars_all = reinterpret_cast<uint64_t*>(slots + (size_t)W * 2 * R * M * rpt);
     const int xitems = ncw_max * p.kp * M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2);  // staging items (upper bound)
-    const bool fused = (MODE == KMODE_W4A4_H) && p.fuse_quant;
+    const bool fused = (MODE != KMODE_W4A16) && p.fuse_quant;
     const int stage_items = fused ? (int)blockDim.x : STAGE_ITEMS;          // items per staging batch
     const int nxb = (xitems + stage_items - 1) / stage_items;
     uint64_t* xbars = bars_all + W * S;
@@ -613,8 +621,8 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
         const int tid = threadIdx.x - W * 32;
         pdl_wait();                                   // the activations come from the previous kernel
         if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, tid, xbars);
-        else if (MODE == KMODE_W4A4_H && p.fuse_quant)
-            stage_x_fused_h<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
+        else if (p.fuse_quant)
+            stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
                                reinterpret_cast<uint32_t*>(fstart + W + 4), reinterpret_cast<float*>(fstart + W + 2));
         else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, tid, xbars);
         return;
@@ -670,7 +678,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
     if (fused)      // consumers take their share of the quantization while their first weight cells are in flight
-        stage_x_fused_h<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
+        stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
                            reinterpret_cast<uint32_t*>(fstart + W + 4), reinterpret_cast<float*>(fstart + W + 2));
     const float gx_raw = (MODE == KMODE_W4A16 || fused) ? 1.0f : __ldg(p.x_gscale);
 
@@ -741,7 +749,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
 
         if (--seg_left == 0) {                                              // segment finished
             float gs = gw_raw;
-            if (MODE == KMODE_W4A4_I8) gs = (gs * gx_raw) * 0.25f;          // ints are 2*e on both sides
+            if (MODE == KMODE_W4A4_I8) gs = (gs * (fused ? *reinterpret_cast<volatile float*>(fstart + W + 2) : gx_raw)) * 0.25f;   // ints are 2*e
             if (MODE == KMODE_W4A4_H)  gs = gs * (fused ? *reinterpret_cast<volatile float*>(fstart + W + 2) : gx_raw);
             const int left = total - f - 1;
             const bool unit_end = (left == 0) ? (x_need - x_items_cell == ncw * x_items_cell) : true;
