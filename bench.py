@@ -415,7 +415,7 @@ def run_ours(args):
 
 # per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from
 # the committed `ncu --set full` capture (profiles/); None until a capture exists for that M.
-TRAFFIC_BYTES_PER_STEP = {1: 278.93e6}    # profiles/r01_ncu_full_m1.md (algorithmic: 274.4 MB)
+TRAFFIC_BYTES_PER_STEP = {1: 279.68e6}    # profiles/r01_ncu_full_m1.md (algorithmic: 274.4 MB)
 
 
 def sweep(wl0, peak):
