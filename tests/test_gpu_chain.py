@@ -11,12 +11,12 @@ import _gpu_util as U
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("M", [1, 4])
-def test_chain_small_dims_every_stage(M):
+@pytest.mark.parametrize("M,fused", [(1, False), (4, False), (1, True), (2, True)])
+def test_chain_small_dims_every_stage(M, fused):
     from paper_2606_13233_b200 import binding as B
     from paper_2606_13233_b200.chain import DecodeChain
     dims = dict(hidden=256, qkv=512, o_in=384, inter=512)
-    ch = DecodeChain(layers=3, M=M, dims=dims, seed=5)
+    ch = DecodeChain(layers=3, M=M, dims=dims, seed=5, fused=fused)
     ch.calibrate(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77)))
     taps = []
     ch.step(taps)
