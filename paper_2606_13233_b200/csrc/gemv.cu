@@ -108,7 +108,8 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     // every consumer warp needs at least one cell of the smallest CTA's flat stream
     const int min_cells = (p.units / ctas) * (p.nch / cfg.ksplit);
     if (p.warps > min_cells) p.warps = min_cells;
-    if (!(gemv_kmode(mode, M) == KMODE_W4A4_H && M == 1) && p.warps > 16) p.warps = 16;             // launch bounds: 1024 threads for M = 1, 640 otherwise
+    const int max_warps = (gemv_max_threads(gemv_kmode(mode, M), M, cfg.rows) - STAGER_THREADS) / 32;   // launch bounds of the instantiation
+    if (p.warps > max_warps) p.warps = max_warps;
     p.units_q = p.units / ctas; p.units_r = p.units % ctas;
     p.cells_q = p.nch / cfg.ksplit; p.cells_r = p.nch % cfg.ksplit;
     dim3 grid(ctas, cfg.ksplit);

@@ -118,6 +118,8 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
+constexpr uint32_t I8_MAGIC_BITS = 0x4B400000u;   // 1.5 * 2^23 = 12582912.0f: ulp 1, integers n with |n| < 2^22 add exactly
+constexpr float    I8_MAGIC      = 12582912.0f;
 __device__ __forceinline__ void decode_x_block(uint2 cw, float sx, uint8_t* base, int half) {
     // nibble -> signed int8 x = 2*e2m1: magnitude LUT through PRMT once per sign, per-byte subtract
     uint32_t out[4];
@@ -135,7 +137,9 @@ __device__ __forceinline__ void decode_x_block(uint2 cw, float sx, uint8_t* base
         }
     }
     *reinterpret_cast<uint4*>(base + half * 16) = make_uint4(out[0], out[1], out[2], out[3]);
-    *reinterpret_cast<int*>(base + 32 + half * 4) = -12 * sum;
+    // the dp4a accumulator starts at MAGIC - 12*sum(x): the finished integer dot, read as FP32 bits, IS the float
+    // 12582912 + dot (exact, |dot| <= 2304), so one packed FADD replaces two I2F (block_pair_w4a4)
+    *reinterpret_cast<int*>(base + 32 + half * 4) = (int)I8_MAGIC_BITS - 12 * sum;
     *reinterpret_cast<float*>(base + 40 + half * 4) = sx;
 }
 
@@ -298,9 +302,33 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
 }
 
 // ---- one 32-k vector (two 16-blocks) of R rows against all M activation rows ------------------
+// packed FP32 helpers (two lanes per instruction; FFMA2 issues at the FFMA rate, _work microbenchmarks)
+__device__ __forceinline__ uint64_t pack2u(uint32_t lo, uint32_t hi) {
+    uint64_t v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "r"(lo), "r"(hi));
+    return v;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t fmul2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t ffma2_i8(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// The two 16-blocks of the vector ride in the two halves of packed FP32 registers: per (row, m)
+// 8 dp4a + FADD2 (remove the magic bias = int->float) + FMUL2 (sW*sX) + FFMA2, instead of
+// 2 I2F + 2 FMUL + 2 FFMA.  accp[r][m] = {sum over even blocks, sum over odd blocks}.
 template <int M, int R>
 __device__ __forceinline__ void block_pair_w4a4(const WLut& lut, const uint4 (&wv)[R], const uint8_t* xbp,
-                                                const float (&sw)[R][8], int j, float (&acc)[R][M]) {
+                                                const uint64_t (&swp)[R][4], int j, uint64_t (&accp)[R][M]) {
     uint32_t u[R][8];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -309,12 +337,13 @@ __device__ __forceinline__ void block_pair_w4a4(const WLut& lut, const uint4 (&w
         decode_w_u8(lut, wv[r].z, u[r][4], u[r][5]);
         decode_w_u8(lut, wv[r].w, u[r][6], u[r][7]);
     }
+    const uint64_t unbias = pack2u(__float_as_uint(-I8_MAGIC), __float_as_uint(-I8_MAGIC));
 #pragma unroll
     for (int m = 0; m < M; ++m) {
         const uint4 xa = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4);
         const uint4 xb = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 16);
         const uint4 ax = *reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4 + 32);
-        const float sx0 = __uint_as_float(ax.z), sx1 = __uint_as_float(ax.w);
+        const uint64_t sx2 = pack2u(ax.z, ax.w);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             int d0 = (int)ax.x, d1 = (int)ax.y;
@@ -322,8 +351,8 @@ __device__ __forceinline__ void block_pair_w4a4(const WLut& lut, const uint4 (&w
             d0 = dp4a_us(u[r][2], xa.z, d0); d0 = dp4a_us(u[r][3], xa.w, d0);
             d1 = dp4a_us(u[r][4], xb.x, d1); d1 = dp4a_us(u[r][5], xb.y, d1);
             d1 = dp4a_us(u[r][6], xb.z, d1); d1 = dp4a_us(u[r][7], xb.w, d1);
-            acc[r][m] = fmaf((float)d0, sw[r][2 * j] * sx0, acc[r][m]);
-            acc[r][m] = fmaf((float)d1, sw[r][2 * j + 1] * sx1, acc[r][m]);
+            const uint64_t dots = fadd2(pack2u((uint32_t)d0, (uint32_t)d1), unbias);
+            accp[r][m] = ffma2_i8(dots, fmul2(swp[r][j], sx2), accp[r][m]);
         }
     }
 }
@@ -572,8 +601,17 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
 // shares, one per consumer warp, so every warp does the same amount of work whatever the shape
 // (a unit cut between warps is recombined in finish_segment).  A warp's bulk-copy ring runs over
 // its whole share and never drains between units.  STAGER_WARPS extra warps decode the activations.
+// threads per CTA the instantiation is compiled for (consumer + stager warps).  R >= 2 tiles per warp keep
+// R x more decoded weights and accumulators live: fewer, fatter warps (<= 8 consumers, 168 registers).
+__host__ __device__ constexpr int gemv_max_threads(int kmode, int M, int R) {
+    if (R >= 2) return 384;
+    if (kmode == KMODE_W4A4_H && M == 1) return 768;
+    if (kmode == KMODE_W4A4_I8 && M >= 7) return 512;     // 12 consumer warps, 128 registers: no spills at M = 7, 8
+    if (kmode == KMODE_W4A4_I8 && M >= 4) return 576;     // 14 consumer warps, 112 registers
+    return 640;
+}
 template <int MODE, int M, int R>
-__global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) gemv_kernel(const GemvParams p) {
+__global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
@@ -688,6 +726,12 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
 #pragma unroll
         for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
 
+    uint64_t accp[R][M];                       // integer path: packed {even blocks, odd blocks} partial sums
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int m = 0; m < M; ++m) accp[r][m] = 0ull;
+
     const WLut lut = make_wlut((uint32_t)p.zero);
     // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
     const size_t xstep = (size_t)p.kp * XVS;
@@ -716,6 +760,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
 #pragma unroll
         for (int hc = 0; hc < CELL_VECS / 4; ++hc) {                       // half cells: 8 scales, 4 vectors
             float sw[R][8];
+            uint64_t swp[R][4];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const uint2 sc = *reinterpret_cast<const uint2*>(st + r * CELL_BYTES + CELL_CODES + lane * (2 * CELL_VECS) + hc * 8);
@@ -725,6 +770,11 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
                 const float2 f3s = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
                 sw[r][0] = f0s.x; sw[r][1] = f0s.y; sw[r][2] = f1s.x; sw[r][3] = f1s.y;
                 sw[r][4] = f2s.x; sw[r][5] = f2s.y; sw[r][6] = f3s.x; sw[r][7] = f3s.y;
+                if (MODE == KMODE_W4A4_I8) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        swp[r][q] = pack2u(__float_as_uint(sw[r][2 * q]), __float_as_uint(sw[r][2 * q + 1]));
+                }
             }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {                                  // 32-k vectors of this lane
@@ -733,7 +783,7 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
                 for (int r = 0; r < R; ++r)
                     wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + (hc * 4 + j) * 512 + lane * 16);
                 const uint8_t* xbp = xlane + (size_t)(hc * 4 + j) * xstep;
-                if (MODE == KMODE_W4A4_I8)     block_pair_w4a4<M, R>(lut, wv, xbp, sw, j, acc);
+                if (MODE == KMODE_W4A4_I8)     block_pair_w4a4<M, R>(lut, wv, xbp, swp, j, accp);
                 else if (MODE == KMODE_W4A4_H) block_pair_w4a4_h<M, R>(wv, xbp, sw, j, acc);
                 else                           block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
             }
@@ -748,6 +798,16 @@ __global__ void __launch_bounds__((MODE == KMODE_W4A4_H && M == 1) ? 768 : 640) 
         if (st == st_end) { st = ring; bar -= (uint32_t)S * 8; phase ^= 1u; }
 
         if (--seg_left == 0) {                                              // segment finished
+            if (MODE == KMODE_W4A4_I8) {
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int m = 0; m < M; ++m) {
+                        const float2 two = unpack2(accp[r][m]);
+                        acc[r][m] = two.x + two.y;
+                        accp[r][m] = 0ull;
+                    }
+            }
             float gs = gw_raw;
             if (MODE == KMODE_W4A4_I8) gs = (gs * (fused ? *reinterpret_cast<volatile float*>(fstart + W + 2) : gx_raw)) * 0.25f;   // ints are 2*e
             if (MODE == KMODE_W4A4_H)  gs = gs * (fused ? *reinterpret_cast<volatile float*>(fstart + W + 2) : gx_raw);
