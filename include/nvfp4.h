@@ -38,7 +38,7 @@
 extern "C" {
 #endif
 
-#define NVFP4_ABI_VERSION 1
+#define NVFP4_ABI_VERSION 2
 
 /* status codes */
 #define NVFP4_OK                      0
@@ -88,11 +88,21 @@ int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx,
 /*
  * Offline weight repack, step a0.  The blob holds exactly the information of the canonical
  * (codes, scales) pair, permuted into the order the GEMV's 128-bit loads consume
- * (4608-byte cells of 32/KP rows x 256*KP k, where the number of K
- * parts KP in {1,2,4,..,32} is a fixed function of (N, K)); rows are padded to a multiple of
- * 32/KP and K to a multiple of 256*KP with zero codes / zero scales (<= 3% extra for K).  nvfp4_repacked_bytes returns 0 for an unsupported shape.
+ * (a 128-byte versioned header {magic "NVF4", ABI version << 16 | KP,
+ * N, K, cell bytes, tiles, cells} followed by 4608-byte cells of 32/KP rows x 256*KP k, where the
+ * number of K parts KP in {1,2,4,..,32} is a fixed function of (N, K) unless overridden with
+ * nvfp4_set_layout_kparts); rows are padded to a multiple of 32/KP and K to a multiple of 256*KP
+ * with zero codes / zero scales (<= 3% extra for K).  nvfp4_repacked_bytes returns 0 for an
+ * unsupported shape.
  *   codes  [device] uint8 [N, K/2];  scales [device] uint8 [N, K/16];  blob_out [device].
  * nvfp4_unpack_weight is the exact inverse (blob -> canonical, byte-identical).
+ * The blob is the library's only persistent artefact: nvfp4_gemv validates the header on the
+ * device against the (N, K, KP, ABI version) of its own call and writes NaN to EVERY output element
+ * if they differ (a stale or foreign blob never yields plausible numbers).
+ * Ordering: nvfp4_gemv starts streaming the blob before it waits for its stream predecessor
+ * (programmatic dependent launch), so the blob must not be WRITTEN by the kernel launched
+ * immediately before nvfp4_gemv on the same stream; nvfp4_repack_weight itself ends with an empty
+ * kernel that makes repack -> gemv safe.
  */
 size_t nvfp4_repacked_bytes(int N, int K);
 int nvfp4_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K,
@@ -113,8 +123,10 @@ int nvfp4_unpack_weight(const void* blob, int N, int K,
  *   x_scales  [device] W4A4 only: uint8 [M, K/16] contiguous;  NULL for W4A16
  *   x_gscale  [device] W4A4 only: one float (e.g. the quantizer's output);  NULL for W4A16
  *   y         [device] out, row m at y + m*ldy elements of y_dtype; ldy >= N
- *   workspace [device] at least nvfp4_gemv_workspace_bytes(M,N,K) bytes: arrival counters and
- *             FP32 split-K partials.  It must be ZERO-FILLED once before its first use; every
+ *   workspace [device] REQUIRED, at least nvfp4_gemv_workspace_bytes(M,N,K) bytes (never 0: the
+ *             weight stream is cut into equal shares per SM wherever that falls, so row tiles at
+ *             the cuts are completed through it): arrival counters and FP32 partials of the
+ *             row tiles cut between CTAs / K slices.  It must be ZERO-FILLED once before its first use; every
  *             call leaves it zero-filled where that matters (the counters), so it can be
  *             reused by any later call on the same stream, and by CUDA-graph replays.  Calls
  *             that may run concurrently need separate workspaces.  The size depends on the
@@ -126,6 +138,17 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
                const void* x, const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx,
                void* y, int y_dtype, int64_t ldy,
                void* workspace, size_t ws_bytes, void* stream);
+
+/*
+ * Per-token (row-wise) activation global scales (R3): the same W4A4 GEMV
+ * with x_gscales = M floats, row m of Y scaled by w_gscale * x_gscales[m].  Feed it from
+ * nvfp4_quantize_act(..., NVFP4_GSCALE_DYNAMIC_PER_ROW): a row's codes then no longer depend on the other
+ * rows of the batch (batch invariance).  Other arguments as for nvfp4_gemv(NVFP4_MODE_W4A4).
+ */
+int nvfp4_gemv_rowscale(const void* w_blob, const float* w_gscale, int N, int K,
+                        const void* x_codes, const uint8_t* x_scales, const float* x_gscales, int M, int64_t ldx,
+                        void* y, int y_dtype, int64_t ldy,
+                        void* workspace, size_t ws_bytes, void* stream);
 
 /*
  * Fused variant of the two calls above: W4A4 GEMV on BF16 activations with the
@@ -144,15 +167,21 @@ int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int
                            void* workspace, size_t ws_bytes, void* stream);
 
 /*
- * Launch-shape override for sweeps (host-side state, not thread-safe; 0 = use the tuned table):
- *   ksplit = number of K ranges (grid.y, 1..64), warps = warps per CTA (1..16),
- *   rows   = 32-row weight tiles per warp, i.e. weight rows per lane (1, 2 or 4),
+ * Launch-shape override for sweeps (process-wide host state behind a mutex; 0 = use the tuned table):
+ *   ksplit = number of K slices (grid.y, 1..64), warps = consumer warps per CTA (1..20),
+ *   rows   = row tiles per warp step (1 or 2; 2 exists for the integer W4A4 path, M >= 2),
  *   stages = depth of each warp's bulk-copy ring (1..16).
- * Returns NVFP4_ERR_INVALID_ARG if out of range.
- * nvfp4_gemv_get_config reports what nvfp4_gemv would use for (mode, M, N, K).
+ * Values the kernels cannot run (shared memory, launch bounds) are clamped; nvfp4_gemv_get_config reports
+ * what nvfp4_gemv would use for (mode, M, N, K).  Returns NVFP4_ERR_INVALID_ARG if out of range.
+ * nvfp4_set_layout_kparts overrides the K-part count KP of the repacked layout (0 = the default function
+ * of (N, K); else a power of two <= 32) for every later size query, repack, unpack and GEMV of this
+ * process; the header records KP, so a blob repacked under another value is rejected (NaN outputs), never
+ * misread.  nvfp4_get_layout_kparts returns the KP in effect for (N, K).
  */
 int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages);
 int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages);
+int nvfp4_set_layout_kparts(int kparts);
+int nvfp4_get_layout_kparts(int N, int K);
 
 /*
  * Glue of the decode chain (step a8, BASELINE.json configs[4]; not part of the paper's kernel):

@@ -24,7 +24,8 @@ ERR_NAMES = {0: "NVFP4_OK", -1: "NVFP4_ERR_INVALID_ARG", -2: "NVFP4_ERR_UNSUPPOR
 # every symbol include/nvfp4.h declares (tests check that the library exports all of them)
 SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp4_repacked_bytes",
            "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
-           "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant")
+           "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant",
+           "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts")
 
 
 class Nvfp4Error(RuntimeError):
@@ -56,6 +57,12 @@ def _load():
     lib.nvfp4_gemv.restype = c_int
     lib.nvfp4_gemv.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64,
                                vp, c_sz, vp]
+    lib.nvfp4_gemv_rowscale.restype = c_int
+    lib.nvfp4_gemv_rowscale.argtypes = [vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp, c_sz, vp]
+    lib.nvfp4_set_layout_kparts.restype = c_int
+    lib.nvfp4_set_layout_kparts.argtypes = [c_int]
+    lib.nvfp4_get_layout_kparts.restype = c_int
+    lib.nvfp4_get_layout_kparts.argtypes = [c_int, c_int]
     lib.nvfp4_gemv_fused_quant.restype = c_int
     lib.nvfp4_gemv_fused_quant.argtypes = [vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_set_config.restype = c_int
@@ -143,6 +150,19 @@ def nvfp4_gemv(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, y=
     return y
 
 
+def nvfp4_gemv_rowscale(w_blob, w_gscale, N, K, x_codes, x_scales, x_gscales, y=None, y_dtype=DTYPE_BF16, workspace=None):
+    """W4A4 GEMV with per-row (per-token) activation global scales x_gscales f32 [M]."""
+    M = x_codes.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x_codes.device)
+    if workspace is None:
+        workspace = new_workspace(M, N, K, x_codes.device)
+    _check(lib.nvfp4_gemv_rowscale(_ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x_codes), _ptr(x_scales), _ptr(x_gscales), M,
+                                   x_codes.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace), workspace.numel(),
+                                   _stream()))
+    return y
+
+
 def nvfp4_gemv_fused_quant(w_blob, w_gscale, N, K, x_bf16, x_gscale_out=None, y=None, y_dtype=DTYPE_BF16,
                            workspace=None):
     """quantize_act + W4A4 gemv in ONE launch; x_bf16 [M,K] torch.bfloat16.  Returns y [M,N]."""
@@ -165,6 +185,14 @@ def nvfp4_gemv_get_config(mode, M, N, K):
     v = [ctypes.c_int(0) for _ in range(4)]
     _check(lib.nvfp4_gemv_get_config(mode, M, N, K, *[ctypes.byref(a) for a in v]))
     return dict(ksplit=v[0].value, warps=v[1].value, rows=v[2].value, stages=v[3].value)
+
+
+def nvfp4_set_layout_kparts(kparts=0):
+    _check(lib.nvfp4_set_layout_kparts(kparts))
+
+
+def nvfp4_get_layout_kparts(N, K) -> int:
+    return lib.nvfp4_get_layout_kparts(N, K)
 
 
 def nvfp4_silu_mul(gu_bf16, h=None):

@@ -3,13 +3,29 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "nvfp4_common.cuh"
 #include "nvfp4_internal.h"
 
 using namespace nvfp4;
 
 static thread_local char g_last_err[256] = "";
-static GemvConfig g_override = {0, 0, 0, 0};      // 0 = use the tuned table
+// process-wide knobs for sweeps (nvfp4_gemv_set_config, nvfp4_set_layout_kparts); 0 = use the tuned table.
+// Guarded by a mutex: a call reads one consistent snapshot.
+static std::mutex g_knob_mutex;
+static GemvConfig g_override = {0, 0, 0, 0};
+static int g_kparts = 0;
+static GemvConfig override_snapshot(int* kp_out) {
+    std::lock_guard<std::mutex> lock(g_knob_mutex);
+    if (kp_out) *kp_out = g_kparts;
+    return g_override;
+}
+static int effective_kparts(int N, int K) {
+    int kp = 0;
+    (void)override_snapshot(&kp);
+    return kp > 0 ? kp : layout_kparts(N, K);
+}
 
 static int cuda_fail(cudaError_t e) {
     snprintf(g_last_err, sizeof(g_last_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
@@ -20,15 +36,14 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 static bool shape_ok(int M, int N, int K) {
     return M >= 1 && M <= 8 && N >= 1 && K >= 16 && (K % 16) == 0 && (int64_t)N * K < ((int64_t)1 << 40);
 }
-static GemvConfig effective_config(int mode, int M, int N, int K) {
-    GemvConfig c = gemv_pick_config(mode, M, N, K);
-    if (g_override.ksplit > 0) c.ksplit = g_override.ksplit;
-    if (g_override.warps > 0) c.warps = g_override.warps;
-    if (g_override.rows > 0) c.rows = g_override.rows;
-    if (g_override.stages > 0) c.stages = g_override.stages;
-    const int nch = make_layout(N, K, layout_kparts(N, K)).ncells;
-    if (c.ksplit > nch) c.ksplit = nch;
-    return c;
+static GemvConfig effective_config(int mode, int M, int N, int K, int kp) {
+    GemvConfig c = gemv_pick_config(mode, M, N, K, kp);
+    const GemvConfig o = override_snapshot(nullptr);
+    if (o.ksplit > 0) c.ksplit = o.ksplit;
+    if (o.warps > 0) c.warps = o.warps;
+    if (o.rows > 0) c.rows = o.rows;
+    if (o.stages > 0) c.stages = o.stages;
+    return gemv_legalize_config(mode, M, N, K, kp, c);
 }
 
 extern "C" {
@@ -53,8 +68,8 @@ int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* c
 
 size_t nvfp4_repacked_bytes(int N, int K) {
     if (!shape_ok(1, N, K)) return 0;
-    const Layout L = make_layout(N, K, layout_kparts(N, K));
-    return (size_t)L.ntiles * L.ncells * CELL_BYTES;
+    const Layout L = make_layout(N, K, effective_kparts(N, K));
+    return (size_t)BLOB_HEADER_BYTES + (size_t)L.ntiles * L.ncells * CELL_BYTES;
 }
 
 int nvfp4_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream) {
@@ -62,7 +77,7 @@ int nvfp4_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int 
     if (!codes || !scales || !blob_out) return NVFP4_ERR_INVALID_ARG;
     if (!shape_ok(1, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     if (!aligned16(codes) || !aligned16(scales) || !aligned16(blob_out)) return NVFP4_ERR_ALIGNMENT;
-    cudaError_t e = launch_repack(codes, scales, N, K, blob_out, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_repack(codes, scales, N, K, effective_kparts(N, K), blob_out, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
@@ -71,21 +86,24 @@ int nvfp4_unpack_weight(const void* blob, int N, int K, uint8_t* codes_out, uint
     if (!codes_out || !scales_out || !blob) return NVFP4_ERR_INVALID_ARG;
     if (!shape_ok(1, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     if (!aligned16(codes_out) || !aligned16(scales_out) || !aligned16(blob)) return NVFP4_ERR_ALIGNMENT;
-    cudaError_t e = launch_unpack(blob, N, K, codes_out, scales_out, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_unpack(blob, N, K, effective_kparts(N, K), codes_out, scales_out, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
 size_t nvfp4_gemv_workspace_bytes(int M, int N, int K) {
     if (!shape_ok(M, N, K)) return 0;
-    const size_t a = gemv_workspace_bytes_for(M, N, K, effective_config(NVFP4_MODE_W4A4, M, N, K));
-    const size_t b = gemv_workspace_bytes_for(M, N, K, effective_config(NVFP4_MODE_W4A16, M, N, K));
-    const size_t c = gemv_workspace_bytes_for(M, N, K, effective_config(MODE_W4A4_FUSED_QUANT, M, N, K));
-    return a > b ? (a > c ? a : c) : (b > c ? b : c);
+    const int kp = effective_kparts(N, K);
+    size_t need = 0;
+    for (int mode : {NVFP4_MODE_W4A4, NVFP4_MODE_W4A16, MODE_W4A4_FUSED_QUANT}) {
+        const size_t b = gemv_workspace_bytes_for(mode, M, N, K, kp, effective_config(mode, M, N, K, kp));
+        need = b > need ? b : need;
+    }
+    return need;
 }
 
-int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K, const void* x,
-               const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
-               int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+static int gemv_common(int mode, const void* w_blob, const float* w_gscale, int N, int K, const void* x,
+                       const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, int64_t ldx, void* y,
+                       int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
     g_last_err[0] = 0;
     if (mode != NVFP4_MODE_W4A4 && mode != NVFP4_MODE_W4A16) return NVFP4_ERR_INVALID_ARG;
     if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
@@ -96,12 +114,27 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
     else                         { if (ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE; }
     if (!aligned16(w_blob) || !aligned16(x) || !aligned16(y) || (workspace && !aligned16(workspace)))
         return NVFP4_ERR_ALIGNMENT;
-    const GemvConfig cfg = effective_config(mode, M, N, K);
-    const size_t need = gemv_workspace_bytes_for(M, N, K, cfg);
-    if (cfg.ksplit > 1 && (!workspace || ws_bytes < need)) return NVFP4_ERR_INVALID_ARG;
-    cudaError_t e = launch_gemv(mode, w_blob, w_gscale, N, K, x, x_scales, x_gscale, M, ldx, y, y_dtype, ldy,
-                                workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));
+    const int kp = effective_kparts(N, K);
+    const GemvConfig cfg = effective_config(mode, M, N, K, kp);
+    const size_t need = gemv_workspace_bytes_for(mode, M, N, K, kp, cfg);
+    if (!workspace || ws_bytes < need) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemv(mode, w_blob, w_gscale, N, K, kp, x, x_scales, x_gscale, gscale_per_row, M, ldx, y, y_dtype,
+                                ldy, workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K, const void* x,
+               const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
+               int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+    return gemv_common(mode, w_blob, w_gscale, N, K, x, x_scales, x_gscale, 0, M, ldx, y, y_dtype, ldy, workspace,
+                       ws_bytes, stream);
+}
+
+int nvfp4_gemv_rowscale(const void* w_blob, const float* w_gscale, int N, int K, const void* x_codes,
+                        const uint8_t* x_scales, const float* x_gscales, int M, int64_t ldx, void* y, int y_dtype,
+                        int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+    return gemv_common(NVFP4_MODE_W4A4, w_blob, w_gscale, N, K, x_codes, x_scales, x_gscales, 1, M, ldx, y, y_dtype, ldy,
+                       workspace, ws_bytes, stream);
 }
 
 int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int K, const void* x_bf16, int M,
@@ -113,25 +146,39 @@ int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int
     if (!shape_ok(M, N, K) || ldy < N || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     if (!aligned16(w_blob) || !aligned16(x_bf16) || !aligned16(y) || (workspace && !aligned16(workspace)))
         return NVFP4_ERR_ALIGNMENT;
-    const GemvConfig cfg = effective_config(MODE_W4A4_FUSED_QUANT, M, N, K);
-    const size_t need = gemv_workspace_bytes_for(M, N, K, cfg);
-    if (cfg.ksplit > 1 && (!workspace || ws_bytes < need)) return NVFP4_ERR_INVALID_ARG;
-    cudaError_t e = launch_gemv(MODE_W4A4_FUSED_QUANT, w_blob, w_gscale, N, K, x_bf16, nullptr, x_gscale_out, M, ldx,
+    const int kp = effective_kparts(N, K);
+    const GemvConfig cfg = effective_config(MODE_W4A4_FUSED_QUANT, M, N, K, kp);
+    const size_t need = gemv_workspace_bytes_for(MODE_W4A4_FUSED_QUANT, M, N, K, kp, cfg);
+    if (!workspace || ws_bytes < need) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemv(MODE_W4A4_FUSED_QUANT, w_blob, w_gscale, N, K, kp, x_bf16, nullptr, x_gscale_out, 0, M, ldx,
                                 y, y_dtype, ldy, workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
 int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages) {
     if (ksplit < 0 || ksplit > 64 || warps < 0 || warps > 20 || stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
-    if (!(rows == 0 || rows == 1 || rows == 2 || rows == 4)) return NVFP4_ERR_INVALID_ARG;
+    if (!(rows == 0 || rows == 1 || rows == 2)) return NVFP4_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_knob_mutex);
     g_override.ksplit = ksplit; g_override.warps = warps; g_override.rows = rows; g_override.stages = stages;
     return NVFP4_OK;
+}
+
+int nvfp4_set_layout_kparts(int kparts) {
+    if (kparts < 0 || kparts > 32 || (kparts & (kparts - 1)) != 0) return NVFP4_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_knob_mutex);
+    g_kparts = kparts;
+    return NVFP4_OK;
+}
+
+int nvfp4_get_layout_kparts(int N, int K) {
+    if (!shape_ok(1, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    return effective_kparts(N, K);
 }
 
 int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages) {
     if (mode != NVFP4_MODE_W4A4 && mode != NVFP4_MODE_W4A16) return NVFP4_ERR_INVALID_ARG;
     if (!shape_ok(M, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
-    const GemvConfig c = effective_config(mode, M, N, K);
+    const GemvConfig c = effective_config(mode, M, N, K, effective_kparts(N, K));
     if (ksplit) *ksplit = c.ksplit;
     if (warps) *warps = c.warps;
     if (rows) *rows = c.rows;

@@ -1,5 +1,6 @@
 // gemv_dispatch.cuh -- runtime (M, R) -> template instantiation.  Included by one .cu per mode so
-// the two families of kernels compile in parallel.
+// the families of kernels compile in parallel.  R = 2 (two row tiles per warp step) is instantiated
+// for the integer path only (gemv_legalize_config never asks for it elsewhere).
 #pragma once
 #include "gemv_kernel.cuh"
 
@@ -7,13 +8,9 @@ namespace nvfp4 {
 
 template <int MODE, int M, int R>
 static cudaError_t launch_one(const GemvParams& p, dim3 grid, int threads, size_t smem, cudaStream_t st) {
-    static size_t configured = 0;                 // per instantiation; grows monotonically
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(gemv_kernel<MODE, M, R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    static size_t configured[MAX_DEVICES] = {};          // per instantiation and device; grows monotonically
+    cudaError_t e = ensure_dynamic_smem(gemv_kernel<MODE, M, R>, configured, smem);
+    if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
     cudaLaunchAttribute attr[1] = {pdl_attribute()};
@@ -23,10 +20,9 @@ static cudaError_t launch_one(const GemvParams& p, dim3 grid, int threads, size_
 
 template <int MODE, int M>
 static cudaError_t launch_r(const GemvParams& p, int R, dim3 grid, int threads, size_t smem, cudaStream_t st) {
-    switch (R) {
-        case 1: return launch_one<MODE, M, 1>(p, grid, threads, smem, st);
-        case 2: return launch_one<MODE, M, 2>(p, grid, threads, smem, st);
-        case 4: return launch_one<MODE, M, 4>(p, grid, threads, smem, st);
+    if (R == 1) return launch_one<MODE, M, 1>(p, grid, threads, smem, st);
+    if constexpr (MODE == KMODE_W4A4_I8) {
+        if (R == 2) return launch_one<MODE, M, 2>(p, grid, threads, smem, st);
     }
     return cudaErrorInvalidValue;
 }

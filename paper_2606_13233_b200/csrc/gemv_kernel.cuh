@@ -2,24 +2,26 @@
 //   Y[m,n] = sum_k vX[m,k] * vW[n,k]     (CUDA cores only)
 //
 // Design (differs from the paper's FP16 cvt+hfma2 kernel):
-//  * lane <-> (weight row, K part): lane = p*(32/KP) + r.  A warp owns R tiles of 32/KP rows and walks
-//    the CTA's K range; the KP lanes of a row take interleaved 32-k vectors and are summed by
-//    log2(KP) warp shuffles ONCE, after the K loop.  KP is a property of the repacked layout
-//    (nvfp4_common.cuh), chosen so that N*KP/32 independent warps fill the GPU: in the tuned
-//    shapes there is no cross-warp and no cross-CTA reduction at all.
-//  * the activations of the K range are decoded ONCE per CTA into shared memory; lanes read
-//    them with LDS.128 (KP distinct addresses per instruction, bank-conflict free).
+//  * lane <-> (weight row, K part): lane = p*(32/KP) + r.  The KP lanes of a row take interleaved 32-k
+//    vectors and are summed by log2(KP) warp shuffles once per segment.  KP is a property of the
+//    repacked layout (nvfp4_common.cuh).
+//  * STREAM-K: the weight of a K slice is one flat stream of `units * cells` 4608-byte cells (unit = R
+//    row tiles, cell = 256*KP k).  The stream is cut into gridDim.x EQUAL shares, one per CTA (about one
+//    CTA per SM), and every CTA's share into W equal shares, one per consumer warp: every SM and every
+//    warp streams the same number of bytes whatever N and K are.  A unit cut between warps is recombined
+//    through shared-memory slots, a unit cut between CTAs (or K slices) through FP32 partials in the
+//    workspace; both are summed in a fixed order by the last contributor to arrive -> deterministic.
+//  * the activations of the CTA's K slice are decoded ONCE per CTA into shared memory by dedicated
+//    stager warps; lanes read them with LDS.128 (KP distinct addresses per instruction, conflict free).
 //  * each warp has a PRIVATE ring of S stages filled by 1-D bulk copies (cp.async.bulk ->
 //    UBLKCP, completion on an mbarrier); lane 0 refills a stage as soon as the warp has read
 //    it.  HBM bytes in flight do not depend on registers or on how fast the math runs.
 //  * W4A4 math is integer and exact inside a 16-block: PRMT byte-LUTs turn 4 nibbles into
 //    4 bytes u = 12 + 2*e (two PRMT, one per sign, OR-ed), dp4a against int8 x = 2*e_x with the
-//    accumulator pre-loaded with -12*sum(x); one I2F + FMUL + FFMA per (row, m, block) applies
-//    sW*sX in FP32.  Cross-block accumulation is FP32 (R8).
-//  * W4A16: cvt.rn.f16x2.e2m1x2 -> FP32, FP32 FMA against FP32 copies of the BF16 activations.
-//  * optional split-K across CTAs (grid.y > 1; only when M*K activations do not fit in shared
-//    memory): FP32 partials in the workspace, summed in fixed order by the last CTA to arrive
-//    (deterministic), which also resets the arrival counter.
+//    accumulator pre-loaded with a magic bias - 12*sum(x); packed FP32 ops apply sW*sX per block pair.
+//    Cross-block accumulation is FP32 (R8).  M = 1 uses cvt.rn.f16x2.e2m1x2 + HFMA2 instead.
+//  * W4A16: cvt.rn.f16x2.e2m1x2 -> FP32, packed FP32 FMA against FP32 copies of the BF16 activations.
+//  * K slices (grid.y > 1) are used only when the M*K activation records do not fit in shared memory.
 #pragma once
 #include "nvfp4_common.cuh"
 #include "nvfp4_internal.h"
@@ -28,25 +30,33 @@
 namespace nvfp4 {
 
 struct GemvParams {
-    const uint8_t* blob;
+    const uint8_t* blob;      // first cell (the 128-byte header precedes it)
     const float* w_gscale;
-    const void* x;            // W4A4: codes (uint8, row stride ldx bytes); W4A16: BF16 bits (row stride ldx elements)
+    const void* x;            // W4A4: codes (uint8, row stride ldx bytes); W4A16 / fused: BF16 bits (row stride ldx elements)
     const uint8_t* x_scales;  // W4A4: [M, K/16]
-    const float* x_gscale;    // W4A4
+    const float* x_gscale;    // W4A4: one float, or M floats (gscale_per_row)
     void* y;
-    float* partials;          // [ksplit][M][Npad]
+    float* partials;          // [ksplit][jmax][M][Npad]
     unsigned int* counters;   // [units], zero on entry, zero on exit
     int64_t ldx, ldy;
-    int N, K, ntiles, nch, Npad;   // tiles of 32/kp rows, cells of 128*kp k, Npad = ntiles * (32/kp)
+    int N, K, ntiles, nch, Npad;   // tiles of 32/kp rows, cells of 256*kp k, Npad = units * R * (32/kp)
     int kp, kp_shift;              // K parts per row inside a warp (power of two) and its log2
     int warps, stages, ksplit;
-    int units;                     // ceil(ntiles / R): work items shared by the gridDim.x CTAs of a K range
-    int units_q, units_r;          // units / gridDim.x and units % gridDim.x   (CTA bx gets q + (bx < r) units)
-    int cells_q, cells_r;          // nch / ksplit and nch % ksplit             (K range by gets q + (by < r) cells)
+    int units;                     // ceil(ntiles / R): a unit = R adjacent row tiles
+    int cells_q, cells_r;          // nch / ksplit and nch % ksplit   (K slice `by` has q + (by < r) cells per unit)
+    // stream-K: slice variant v (0: cells_q cells per unit, 1: cells_q + 1) has T_v = units * cells flat cells;
+    // CTA b of gridDim.x owns [start_v(b), start_v(b+1)), start_v(b) = b*share_q[v] + (b*share_r[v]) / gridDim.x
+    int share_q[2], share_r[2];
+    float inv_share[2];            // gridDim.x / T_v (estimate for the inverse of start_v)
+    int jmax;                      // max number of CTAs of one slice that share a unit (partials slots)
+    int ucta_max;                  // max number of units a CTA touches
+    int nxb;                       // staging-batch mbarriers
     int y_bf16;
     int zero;                      // always 0 (see make_wlut)
     int fuse_quant;                // x is BF16 [M,K] (ldx elements): quantise it inside the kernel (W4A4 modes)
+    int gscale_per_row;            // x_gscale holds M per-row (per-token) global scales
     float* x_gscale_out;           // fuse_quant: optional device float that receives the activation global scale
+    uint4 hdr_expect;              // blob_header_words(N, K, kp)
 };
 
 // shared-memory bytes of activations per 32-k block pair and per m
@@ -198,7 +208,7 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
 // pass 1: tensor-wide amax of the BF16 activations (whole [M,K], every CTA redundantly: <= 410 KB from L2),
 // pass 2: per 16-block the R2 sequence of quant_block.cuh, then straight to the f16 record (the E2M1 code is
 // produced by cvt.rn.satfinite.e2m1x2.f32 and expanded by cvt.rn.f16x2.e2m1x2, so the values are exactly
-// those of quantize_act followed by the normal staging).  `red` = 8 words of shared memory.
+// those of quantize_act followed by the normal staging).  `red` = one word per warp of the CTA (32 reserved in the shared-memory map).
 template <int M, bool HALF>
 __device__ __forceinline__ void stage_x_fused(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
                                                 uint64_t* xbars, uint32_t* red, float* gx_slot) {
@@ -476,45 +486,103 @@ __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uin
     }
 }
 
-// ---- a7: write one finished unit (R tiles); `acc` holds the unit's complete sums over this CTA's
-// K range in the writer lanes (part == 0).  With split K across CTAs (grid.y > 1) the FP32 partial
-// goes to the workspace and the last warp to arrive for this unit sums all K ranges in fixed order.
+// ---- shared-memory carve-up: ONE definition for the host (gemv_smem_bytes) and the kernel -----------
+struct SmemMap { uint32_t xs, ring, slots, bars, xbars, cnt, fstart, cstart, misc, total; };
+__host__ __device__ inline SmemMap gemv_smem_map(int kmode, int M, int R, int W, int S, int rpt, int ncw_max, int kp,
+                                                 int nxb, int ucta_max, int nb) {
+    SmemMap m;
+    uint32_t o = 0;
+    m.xs = o;     o += ((uint32_t)ncw_max * CELL_VECS * kp * xvec_stride(kmode, M) + 127u) & ~127u;   // activation records
+    m.ring = o;   o += (uint32_t)W * S * R * CELL_BYTES;                   // per-warp bulk-copy rings
+    m.slots = o;  o += (uint32_t)W * 2 * R * M * rpt * 4;                  // segment partials (two per warp)
+    m.bars = o;   o += (uint32_t)W * S * 8;                                // ring mbarriers
+    m.xbars = o;  o += (uint32_t)nxb * 8;                                  // staging-batch mbarriers
+    m.cnt = o;    o += (uint32_t)ucta_max * 4;                             // per-unit arrival counters (warps)
+    m.fstart = o; o += (uint32_t)(W + 1) * 4;                              // warp share starts
+    m.cstart = o; o += (uint32_t)2 * (nb + 1) * 4;                         // CTA share starts, both slice variants
+    m.misc = o;   o += (2 + 32) * 4;                                       // fused quantizer: gX slot + per-warp amax
+    m.total = (o + 15u) & ~15u;
+    return m;
+}
+
+// CTA-constant context of the stream-K bookkeeping
+struct CtaCtx {
+    int ncw;            // cells per unit in this CTA's K slice
+    int o, L;           // the CTA's share in local coordinates: cells [o, o + L), unit boundaries at multiples of ncw
+    int ub;             // global index of local unit 0
+    int var;            // slice variant (0: cells_q, 1: cells_q + 1 cells per unit)
+    int nb;             // CTAs per slice
+    const int* cstart;  // [2][nb + 1] share starts per variant
+};
+
+// CTAs of a variant-v slice whose share intersects unit `unit`: [lo, hi].  start_v(b) is non-decreasing
+// with start_v(0) = 0; the float estimate is corrected against the table.
+__device__ __forceinline__ void contrib_range(const GemvParams& p, const CtaCtx& c, int v, int unit, int& lo, int& hi) {
+    const int ncw_v = p.cells_q + v;
+    const int* cs = c.cstart + v * (c.nb + 1);
+    const int x0 = unit * ncw_v, x1 = x0 + ncw_v - 1;
+    int b = (int)((float)x0 * p.inv_share[v]);
+    b = b < 0 ? 0 : (b > c.nb - 1 ? c.nb - 1 : b);
+    while (b + 1 < c.nb && cs[b + 1] <= x0) ++b;
+    while (cs[b] > x0) --b;
+    lo = b;
+    while (b + 1 < c.nb && cs[b + 1] <= x1) ++b;
+    hi = b;
+}
+
+// ---- a7: write one finished unit (R tiles); `acc` holds the CTA's complete sums for the unit over its
+// cells in the writer lanes (part == 0).  If the CTA does not hold the unit's whole K range (the stream-K cut
+// fell inside the unit, or K is sliced across grid.y) the FP32 partial goes to the workspace and the last
+// CTA to arrive for this unit sums all contributions in a fixed order (slice-major, then CTA order).
 template <int M, int R>
-__device__ __forceinline__ void emit_unit(const GemvParams& p, float (&acc)[R][M], int unit, int lane, bool writer,
-                                          int rsub, int rpt, float gs) {
+__device__ __forceinline__ void emit_unit(const GemvParams& p, const CtaCtx& c, float (&acc)[R][M], int ul, int lane,
+                                          bool writer, int rsub, int rpt, float gs) {
+    const int unit = c.ub + ul;
     int nvalid = p.ntiles - unit * R;
     nvalid = nvalid > R ? R : nvalid;
-    if (p.ksplit > 1) {
+    const bool cta_whole = (p.ksplit == 1) && (ul * c.ncw >= c.o) && ((ul + 1) * c.ncw <= c.o + c.L);
+    if (!cta_whole) {
+        int lo0 = 0, hi0 = -1, lo1 = 0, hi1 = -1;
+        const int nvar1 = p.cells_r, nvar0 = p.ksplit - p.cells_r;          // slices per variant
+        if (nvar0 > 0) contrib_range(p, c, 0, unit, lo0, hi0);
+        if (nvar1 > 0) contrib_range(p, c, 1, unit, lo1, hi1);
+        const int myslot = (int)blockIdx.y * p.jmax + ((int)blockIdx.x - (c.var ? lo1 : lo0));
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int n = (unit * R + r) * rpt + rsub;
             if (writer && r < nvalid) {
 #pragma unroll
                 for (int m = 0; m < M; ++m)
-                    __stcg(p.partials + ((int64_t)blockIdx.y * M + m) * p.Npad + n, acc[r][m]);
+                    __stcg(p.partials + ((int64_t)myslot * M + m) * p.Npad + n, acc[r][m]);
             }
         }
         __threadfence();
         __syncwarp();
         unsigned int last = 0;
         if (lane == 0) {
+            const unsigned int expected = (unsigned int)(nvar0 * (hi0 - lo0 + 1) + nvar1 * (hi1 - lo1 + 1));
             const unsigned int old = atomicAdd(p.counters + unit, 1u);
-            last = (old == (unsigned int)p.ksplit - 1u);
+            last = (old == expected - 1u);
             if (last) p.counters[unit] = 0u;                              // leave the workspace clean
         }
         last = __shfl_sync(0xFFFFFFFFu, last, 0);
         if (!last) return;
         __threadfence();
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int n = (unit * R + r) * rpt + rsub;
-            if (writer && r < nvalid) {
+        for (int r = 0; r < R; ++r)
 #pragma unroll
-                for (int m = 0; m < M; ++m) {
-                    float sum = 0.0f;
-                    for (int ks = 0; ks < p.ksplit; ++ks)
-                        sum += __ldcg(p.partials + ((int64_t)ks * M + m) * p.Npad + n);
-                    acc[r][m] = sum;
+            for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
+        for (int ks = 0; ks < p.ksplit; ++ks) {
+            const int nj = ks < p.cells_r ? (hi1 - lo1) : (hi0 - lo0);
+            for (int j = 0; j <= nj; ++j) {
+                const float* src = p.partials + (int64_t)(ks * p.jmax + j) * M * p.Npad;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const int n = (unit * R + r) * rpt + rsub;
+                    if (writer && r < nvalid) {
+#pragma unroll
+                        for (int m = 0; m < M; ++m) acc[r][m] += __ldcg(src + (int64_t)m * p.Npad + n);
+                    }
                 }
             }
         }
@@ -525,7 +593,8 @@ __device__ __forceinline__ void emit_unit(const GemvParams& p, float (&acc)[R][M
         if (writer && r < nvalid && n < p.N) {
 #pragma unroll
             for (int m = 0; m < M; ++m) {
-                const float v = acc[r][m] * gs;
+                // per-token activation scales (nvfp4_gemv_rowscale): gs holds the weight-side factor only
+                const float v = acc[r][m] * (p.gscale_per_row ? gs * __ldg(p.x_gscale + m) : gs);
                 if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
                 else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
             }
@@ -533,17 +602,16 @@ __device__ __forceinline__ void emit_unit(const GemvParams& p, float (&acc)[R][M
     }
 }
 
-// first cell of consumer warp w's share of the CTA's flat stream of T cells (W <= T <= 2^26)
-__device__ __forceinline__ int flat_start(int w, int T, int W) { return (int)(((unsigned)w * (unsigned)T) / (unsigned)W); }
+// first cell of consumer warp w's share of the CTA's L cells (W <= L <= 2^26)
+__device__ __forceinline__ int flat_start(int w, int L, int W) { return (int)(((unsigned)w * (unsigned)L) / (unsigned)W); }
 
-// ---- a6: a warp finished its segment [cells seg_c0 .. seg_c1] of unit `ul` (CTA-local index).
-// K parts of a row are summed by shuffles; a unit shared by several warps is combined through
-// shared-memory slots (two per warp: slot 0 = the segment that starts the warp's share, slot 1 =
-// any later one) by the LAST warp to arrive, in fixed warp order -> deterministic.
+// ---- a6: a warp finished its segment of local unit `ul`.  K parts of a row are summed by shuffles; a
+// unit shared by several warps is combined through shared-memory slots (two per warp: slot 0 = the
+// segment that starts the warp's share, slot 1 = any later one) by the LAST warp to arrive, in fixed
+// warp order -> deterministic.
 template <int M, int R>
-__device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)[R][M], float* slots, int* cnt,
-                                               const int* fstart,
-                                               int ul, int unit, bool whole, bool seg_at_share_start, int ncw, int T,
+__device__ __forceinline__ void finish_segment(const GemvParams& p, const CtaCtx& c, float (&acc)[R][M], float* slots,
+                                               int* cnt, const int* fstart, int ul, bool whole, bool seg_at_share_start,
                                                int warp, int lane, int part, int rsub, int rpt, float gs) {
     for (int off = rpt; off < 32; off <<= 1) {                  // lanes of one row are rpt apart
 #pragma unroll
@@ -562,8 +630,9 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
 #pragma unroll
                 for (int m = 0; m < M; ++m) mine[(r * M + m) * rpt + rsub] = acc[r][m];
         }
-        // contributors of this unit: warps whose share intersects [ul*ncw, (ul+1)*ncw)
-        const int lo = ul * ncw, hi = lo + ncw - 1;
+        // contributors of this unit: warps whose share intersects [ul*ncw, (ul+1)*ncw)  (fstart[0] = o, so a
+        // unit that begins before the CTA's share starts at warp 0; one that ends after it ends at warp W-1)
+        const int lo = ul * c.ncw, hi = lo + c.ncw - 1;
         int w_first = 0, w_last = 0;
         for (int w = 0; w < W; ++w) {
             const int fs = fstart[w];
@@ -593,23 +662,18 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, float (&acc)
             }
         }
     }
-    emit_unit<M, R>(p, acc, unit, lane, writer, rsub, rpt, gs);
+    emit_unit<M, R>(p, c, acc, ul, lane, writer, rsub, rpt, gs);
 }
 
-// Persistent and statically balanced.  gridDim.x CTAs (about one per SM) share the `units` (R tiles
-// each) evenly; inside a CTA the flat stream of T = units_cta * ncw cells is cut into W equal
-// shares, one per consumer warp, so every warp does the same amount of work whatever the shape
-// (a unit cut between warps is recombined in finish_segment).  A warp's bulk-copy ring runs over
-// its whole share and never drains between units.  STAGER_WARPS extra warps decode the activations.
-// threads per CTA the instantiation is compiled for (consumer + stager warps).  R >= 2 tiles per warp keep
-// R x more decoded weights and accumulators live: fewer, fatter warps (<= 8 consumers, 168 registers).
+// threads per CTA the instantiation is compiled for (consumer + stager warps)
 __host__ __device__ constexpr int gemv_max_threads(int kmode, int M, int R) {
-    if (R >= 2) return 384;
-    if (kmode == KMODE_W4A4_H && M == 1) return 768;
-    if (kmode == KMODE_W4A4_I8 && M >= 7) return 512;     // 12 consumer warps, 128 registers: no spills at M = 7, 8
-    // (M = 4..6 at 576 threads / 14 consumer warps measured 8-18 % slower than 16 warps at 96 registers)
+    if (kmode == KMODE_W4A4_H && M == 1 && R == 1) return 768;
+    if (R >= 2) return 512;                               // 12 consumer warps, 128 registers
+    if (kmode == KMODE_W4A4_I8 && M >= 7) return 512;     // 128 registers: no spills at M = 7, 8
     return 640;
 }
+
+// Persistent, stream-K balanced (see the file header).  STAGER_WARPS extra warps decode the activations.
 template <int MODE, int M, int R>
 __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -618,39 +682,50 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const int rsub = lane & ((32 >> p.kp_shift) - 1), part = lane >> (5 - p.kp_shift);   // lane = part*rpt + rsub
     const int rpt = 32 >> p.kp_shift;
     constexpr int XBP = xbp_bytes(MODE);
+    (void)XBP;
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
 
-    // K range of this CTA (whole cells of 128*kp k)
-    // (quotients and remainders come from the host: no integer division in the prologue)
-    const int by = blockIdx.y, bx = blockIdx.x;
+    // K slice of this CTA (whole cells of 256*kp k); quotients and remainders come from the host
+    const int by = blockIdx.y, bx = blockIdx.x, nb = gridDim.x;
+    CtaCtx c;
+    c.var = by < p.cells_r ? 1 : 0;
+    c.nb = nb;
     const int c0 = by * p.cells_q + (by < p.cells_r ? by : p.cells_r);
-    const int ncw = p.cells_q + (by < p.cells_r ? 1 : 0);
+    const int ncw = p.cells_q + c.var;
+    c.ncw = ncw;
     const int ncw_max = p.cells_q + (p.cells_r > 0 ? 1 : 0);
+    // this CTA's equal share [F0, F1) of the slice's flat stream of units * ncw cells
+    const unsigned F0 = (unsigned)bx * (unsigned)p.share_q[c.var] + ((unsigned)bx * (unsigned)p.share_r[c.var]) / (unsigned)nb;
+    const unsigned F1 = (unsigned)(bx + 1) * (unsigned)p.share_q[c.var] + ((unsigned)(bx + 1) * (unsigned)p.share_r[c.var]) / (unsigned)nb;
+    c.L = (int)(F1 - F0);
+    c.ub = (int)(F0 / (unsigned)ncw);
+    c.o = (int)(F0 - (unsigned)c.ub * (unsigned)ncw);
+    const int L = c.L;
 
-    // units of this CTA
-    const int u0 = bx * p.units_q + (bx < p.units_r ? bx : p.units_r);
-    const int u1 = u0 + p.units_q + (bx < p.units_r ? 1 : 0);
-    const int ucta_max = p.units_q + (p.units_r > 0 ? 1 : 0);
-    const int T = (u1 - u0) * ncw;                                          // cells of this CTA (>= W)
-
-    // shared memory carve-up (must match gemv_smem_bytes)
-    uint8_t* xs = smem;                                                      // activations
+    const SmemMap map = gemv_smem_map(MODE, M, R, W, S, rpt, ncw_max, p.kp, p.nxb, p.ucta_max, nb);
+    uint8_t* xs = smem + map.xs;                                             // activations
     constexpr int XVS = xvec_stride(MODE, M);
-    const size_t xs_bytes = ((size_t)ncw_max * CELL_VECS * p.kp * XVS + 127) & ~(size_t)127;
-    uint8_t* ring_all = smem + xs_bytes;
-    float* slots = reinterpret_cast<float*>(ring_all + (size_t)W * S * STAGE_BYTES);
-    uint64_t* bars_all = reinterpret_cast<uint64_t*>(slots + (size_t)W * 2 * R * M * rpt);
-    const int xitems = ncw_max * p.kp * M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2);  // staging items (upper bound)
+    uint8_t* ring_all = smem + map.ring;
+    float* slots = reinterpret_cast<float*>(smem + map.slots);
+    uint64_t* bars_all = reinterpret_cast<uint64_t*>(smem + map.bars);
+    uint64_t* xbars = reinterpret_cast<uint64_t*>(smem + map.xbars);
+    int* cnt = reinterpret_cast<int*>(smem + map.cnt);
+    int* fstart = reinterpret_cast<int*>(smem + map.fstart);
+    int* cstart = reinterpret_cast<int*>(smem + map.cstart);
+    float* gx_slot = reinterpret_cast<float*>(smem + map.misc);
+    uint32_t* red = reinterpret_cast<uint32_t*>(smem + map.misc) + 2;
+    c.cstart = cstart;
     const bool fused = (MODE != KMODE_W4A16) && p.fuse_quant;
     const int stage_items = fused ? (int)blockDim.x : STAGE_ITEMS;          // items per staging batch
-    const int nxb = (xitems + stage_items - 1) / stage_items;
-    uint64_t* xbars = bars_all + W * S;
-    int* cnt = reinterpret_cast<int*>(xbars + nxb);
-    int* fstart = cnt + ucta_max;
 
-    for (int i = threadIdx.x; i < ucta_max; i += blockDim.x) cnt[i] = 0;
-    if (threadIdx.x <= W) fstart[threadIdx.x] = flat_start(threadIdx.x, T, W);
-    for (int i = threadIdx.x; i < nxb; i += blockDim.x)
+    for (int i = threadIdx.x; i < p.ucta_max; i += blockDim.x) cnt[i] = 0;
+    if (threadIdx.x <= W) fstart[threadIdx.x] = c.o + flat_start(threadIdx.x, L, W);
+    if (threadIdx.x <= nb) {                                                // blockDim.x >= 160 > nb
+        const unsigned b = threadIdx.x;
+        cstart[b] = (int)(b * (unsigned)p.share_q[0] + (b * (unsigned)p.share_r[0]) / (unsigned)nb);
+        cstart[nb + 1 + b] = (int)(b * (unsigned)p.share_q[1] + (b * (unsigned)p.share_r[1]) / (unsigned)nb);
+    }
+    for (int i = threadIdx.x; i < p.nxb; i += blockDim.x)
         mbar_init(smem_u32(xbars + i), fused ? blockDim.x : STAGER_THREADS);
     if (threadIdx.x == 0) mbar_fence_init();
     __syncthreads();
@@ -660,8 +735,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         pdl_wait();                                   // the activations come from the previous kernel
         if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, tid, xbars);
         else if (p.fuse_quant)
-            stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
-                               reinterpret_cast<uint32_t*>(fstart + W + 4), reinterpret_cast<float*>(fstart + W + 2));
+            stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
         else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, tid, xbars);
         return;
     }
@@ -675,7 +749,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
 
     // producer cursor (used by lane 0 only): next cell to request.  Within a unit the cells of a
-    // tile are contiguous in the blob; with ksplit == 1 and R == 1 the whole share is one run.
+    // tile are contiguous in the blob; with one K slice and R == 1 the whole share is one run.
     const bool leader = (lane == 0);
     int p_left = 0, p_count = 0, p_nv = 0;
     uint32_t p_dst = smem_u32(ring), p_bar = smem_u32(bars);
@@ -683,7 +757,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const uint8_t* p_src = nullptr;
     {
         const int ul = f0_ul, cell = f0 - ul * ncw;
-        const int tile0 = (u0 + ul) * R;
+        const int tile0 = (c.ub + ul) * R;
         p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
         p_left = ncw - cell;
         p_nv = p.ntiles - tile0; p_nv = p_nv > R ? R : p_nv;
@@ -704,11 +778,13 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         p_dst += STAGE_BYTES; p_bar += 8;
         if (p_dst == ring_end) { p_dst -= (uint32_t)S * STAGE_BYTES; p_bar -= (uint32_t)S * 8; }
     };
+    uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
     if (leader) {                                                           // start the weight stream first
         for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
         mbar_fence_init();
         const int npre = total < S ? total : S;
         for (int i = 0; i < npre; ++i) issue();
+        hdr = __ldg(reinterpret_cast<const uint4*>(p.blob - BLOB_HEADER_BYTES));    // checked before the first output
     }
     // the weight stream is under way; everything below touches data of the previous kernel
     pdl_wait();
@@ -716,9 +792,8 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
     if (fused)      // consumers take their share of the quantization while their first weight cells are in flight
-        stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars,
-                           reinterpret_cast<uint32_t*>(fstart + W + 4), reinterpret_cast<float*>(fstart + W + 2));
-    const float gx_raw = (MODE == KMODE_W4A16 || fused) ? 1.0f : __ldg(p.x_gscale);
+        stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
+    const float gx_raw = (MODE == KMODE_W4A16 || fused || p.gscale_per_row) ? 1.0f : __ldg(p.x_gscale);
 
     float acc[R][M];
 #pragma unroll
@@ -733,7 +808,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         for (int m = 0; m < M; ++m) accp[r][m] = 0ull;
 
     const WLut lut = make_wlut((uint32_t)p.zero);
-    // this lane's activation records: vector (cell*4 + j)*kp + part  ->  stride between j steps = kp records
+    // this lane's activation records: vector (cell*8 + j)*kp + part  ->  stride between j steps = kp records
     const size_t xstep = (size_t)p.kp * XVS;
     const uint8_t* xlane0 = xs + (size_t)part * XVS;
     int c_ul = f0_ul;
@@ -752,7 +827,11 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     int x_need = (cell0 + 1) * x_items_cell;                                // items that must be staged
     int x_have = 0;                                                         // items known to be staged
     uint32_t xbar = smem_u32(xbars);
-    __syncwarp();
+    // a blob that was not repacked for this (N, K, KP, ABI version) must not produce plausible numbers: NaN outputs
+    hdr.x = __shfl_sync(0xFFFFFFFFu, hdr.x, 0); hdr.y = __shfl_sync(0xFFFFFFFFu, hdr.y, 0);
+    hdr.z = __shfl_sync(0xFFFFFFFFu, hdr.z, 0); hdr.w = __shfl_sync(0xFFFFFFFFu, hdr.w, 0);
+    const bool blob_ok = (hdr.x == p.hdr_expect.x) && (hdr.y == p.hdr_expect.y) && (hdr.z == p.hdr_expect.z) &&
+                         (hdr.w == p.hdr_expect.w);
     for (int f = 0; f < total; ++f) {
         while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += stage_items; }
         mbar_wait(bar, phase);
@@ -809,11 +888,12 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
                     }
             }
             float gs = gw_raw;
-            if (MODE == KMODE_W4A4_I8) gs = (gs * (fused ? *reinterpret_cast<volatile float*>(fstart + W + 2) : gx_raw)) * 0.25f;   // ints are 2*e
-            if (MODE == KMODE_W4A4_H)  gs = gs * (fused ? *reinterpret_cast<volatile float*>(fstart + W + 2) : gx_raw);
+            if (MODE == KMODE_W4A4_I8) gs = (gs * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw)) * 0.25f;   // ints are 2*e
+            if (MODE == KMODE_W4A4_H)  gs = gs * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw);
+            if (!blob_ok) gs = __int_as_float(0x7FC00000);
             const int left = total - f - 1;
             const bool unit_end = (left == 0) ? (x_need - x_items_cell == ncw * x_items_cell) : true;
-            finish_segment<M, R>(p, acc, slots, cnt, fstart, c_ul, u0 + c_ul, seg_from0 && unit_end, seg_first, ncw, T,
+            finish_segment<M, R>(p, c, acc, slots, cnt, fstart, c_ul, seg_from0 && unit_end, seg_first,
                                  warp, lane, part, rsub, rpt, gs);
 #pragma unroll
             for (int r = 0; r < R; ++r)

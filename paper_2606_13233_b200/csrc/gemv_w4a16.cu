@@ -1,4 +1,4 @@
-// gemv_w4a16.cu -- instantiates the KMODE_W4A16 GEMV kernels (all M = 1..8, R = 1, 2, 4).
+// gemv_w4a16.cu -- instantiates the KMODE_W4A16 GEMV kernels (all M = 1..8, R = 1).
 #include "gemv_dispatch.cuh"
 
 namespace nvfp4 {

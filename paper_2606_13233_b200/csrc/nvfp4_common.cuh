@@ -6,7 +6,6 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include <stdlib.h>
 
 #include "../../include/nvfp4.h"
 
@@ -18,18 +17,33 @@ namespace nvfp4 {
 
 // ---- repacked weight blob geometry -------------------------
 // A lane of the GEMV owns (row r, K part p): lane = p*(32/KP) + r (lanes of one K part are adjacent,
-// so their activation loads hit one address per part), KP = 2^i K parts per row inside a
-// warp (chosen per weight shape by layout_kparts, so that N*KP/32 independent warp units fill
-// the 148 SMs without any cross-warp or cross-CTA reduction).  A "cell" is what one warp consumes
-// in CELL_VECS = 8 128-bit loads per lane: 32/KP weight rows x 256*KP consecutive k:
+// so their activation loads hit one address per part), KP = 2^i K parts per row inside a warp
+// (chosen per weight shape by layout_kparts, or given explicitly to nvfp4_repack_weight_kp).
+// A "cell" is what one warp consumes in CELL_VECS = 8 128-bit loads per lane: 32/KP weight rows x
+// 256*KP consecutive k:
 //   bytes [0,4096)    codes:  vector j (0..7), lane (r,p) -> 16 B = the 32 k starting at
 //                             cell_k0 + (j*KP + p)*32 of row tile_row0 + r
 //   bytes [4096,4608) scales: lane (r,p) -> 16 B = the E4M3 scales of those 8 x 2 blocks (j-major)
-// Blob = cells in [tile = n/(32/KP)][cell = k/(256*KP)] order, so one warp streams a contiguous run.
+// Blob = 128-byte header, then the cells in [tile = n/(32/KP)][cell = k/(256*KP)] order, so one warp
+// streams a contiguous run.
 constexpr int CELL_VECS   = 8;                          // 128-bit code vectors per lane and cell
 constexpr int CELL_CODES  = CELL_VECS * 512;            // 4096
 constexpr int CELL_SCALES = CELL_VECS * 64;             // 512
 constexpr int CELL_BYTES  = CELL_CODES + CELL_SCALES;   // 4608 = 0.5625 B per weight
+
+// Versioned blob header (the only persistent artefact of the library).  The GEMV
+// compares the first four words with what its launch expects and writes NaN outputs on a mismatch.
+constexpr int      BLOB_HEADER_BYTES = 128;             // keeps the cells 128-byte aligned
+constexpr uint32_t BLOB_MAGIC        = 0x3446564Eu;     // "NVF4"
+struct BlobHeader {
+    uint32_t magic;          // BLOB_MAGIC
+    uint32_t version_kp;     // NVFP4_ABI_VERSION << 16 | KP
+    uint32_t N, K;
+    uint32_t cell_bytes, ntiles, ncells, reserved;
+};
+__host__ __device__ inline uint4 blob_header_words(int N, int K, int kp) {
+    return make_uint4(BLOB_MAGIC, ((uint32_t)NVFP4_ABI_VERSION << 16) | (uint32_t)kp, (uint32_t)N, (uint32_t)K);
+}
 
 struct Layout {
     int kp;         // K parts per row inside a warp (1, 2, 4, 8, 16 or 32)
@@ -47,16 +61,11 @@ __host__ __device__ inline Layout make_layout(int N, int K, int kp) {
     return L;
 }
 
-// K parts for a weight shape: the smallest power of two that yields >= 296 (= 2 per SM) tiles of at most
-// 32 cells each, among those whose K padding costs at most 3% more than KP = 1 does.  (Balance inside an SM comes from the
-// in-CTA stream split, so few K parts are needed; fewer parts = more uniform activation loads.)
+// Default K parts for a weight shape: the smallest power of two that yields >= 296 (= 2 per SM) tiles of
+// at most 32 cells each, among those whose K padding costs at most 3% more than KP = 1 does.  (Balance
+// across and inside the SMs comes from the flat-stream split of the GEMV, so few K parts are needed;
+// fewer parts = more uniform activation loads.)
 __host__ __device__ inline int layout_kparts(int N, int K) {
-#ifndef __CUDA_ARCH__
-    {   // experiments only (read once): NVFP4_KP forces the K-part count of the layout
-        static const int forced = [] { const char* e = getenv("NVFP4_KP"); return e ? atoi(e) : 0; }();
-        if (forced > 0) return forced;
-    }
-#endif
     const long long ck1 = 32 * CELL_VECS;
     const long long pad1 = ((K + ck1 - 1) / ck1) * ck1;
     int best = 1;

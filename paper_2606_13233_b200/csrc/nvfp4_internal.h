@@ -12,10 +12,10 @@ constexpr int MODE_W4A4_FUSED_QUANT = 2;
 
 // launch shape of the GEMV: every field > 0
 struct GemvConfig {
-    int warps;    // warps per CTA, each owns `rows` row tiles (32 rows each) -> no cross-warp reduce
-    int rows;     // R: row tiles (32/KP rows each) per warp (1, 2 or 4)
-    int stages;   // depth of each warp's private bulk-copy ring (cells of 4608 B per tile)
-    int ksplit;   // number of K ranges (grid.y); > 1 -> partials through the workspace
+    int warps;    // consumer warps per CTA; each streams an equal share of the CTA's cells
+    int rows;     // R: row tiles (32/KP rows each) per warp step (1 or 2): x records are loaded once per R tiles
+    int stages;   // depth of each warp's private bulk-copy ring (R cells of 4608 B per stage)
+    int ksplit;   // number of K slices (grid.y); each slice's activations are staged by its own CTAs
 };
 
 // launch attribute that lets a kernel start before its stream predecessor has finished (PDL)
@@ -26,18 +26,38 @@ inline cudaLaunchAttribute pdl_attribute() {
     return a;
 }
 
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: remember the largest value set per
+// (kernel, device) so that a process driving several GPUs opts every one of them in.
+constexpr int MAX_DEVICES = 64;
+template <typename Kernel>
+inline cudaError_t ensure_dynamic_smem(Kernel kernel, size_t* configured /*[MAX_DEVICES]*/, size_t smem) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem > __atomic_load_n(&configured[dev], __ATOMIC_RELAXED)) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        __atomic_store_n(&configured[dev], smem, __ATOMIC_RELAXED);     // racing threads at worst set it twice
+    }
+    return cudaSuccess;
+}
+
 cudaError_t launch_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* codes, uint8_t* scales,
                                 float* gscale, int gscale_mode, cudaStream_t st);
+cudaError_t launch_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, uint8_t* scales, float* gscale,
+                                     int gscale_mode, void* h_bf16_opt, cudaStream_t st);
 
-cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob, cudaStream_t st);
-cudaError_t launch_unpack(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st);
+cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, int K, int kp, void* blob, cudaStream_t st);
+cudaError_t launch_unpack(const void* blob, int N, int K, int kp, uint8_t* codes, uint8_t* scales, cudaStream_t st);
 
-GemvConfig gemv_pick_config(int mode, int M, int N, int K);
-size_t gemv_workspace_bytes_for(int M, int N, int K, const GemvConfig& c);
-size_t gemv_smem_bytes(int mode, int M, int N, int K, const GemvConfig& c);
-cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, const void* x,
-                        const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
-                        int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st);
+GemvConfig gemv_pick_config(int mode, int M, int N, int K, int kp);
+GemvConfig gemv_legalize_config(int mode, int M, int N, int K, int kp, GemvConfig c);
+size_t gemv_workspace_bytes_for(int mode, int M, int N, int K, int kp, const GemvConfig& c);
+size_t gemv_smem_bytes(int mode, int M, int N, int K, int kp, const GemvConfig& c);
+cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, int kp, const void* x,
+                        const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, int64_t ldx, void* y,
+                        int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st);
 
 cudaError_t launch_silu_mul(const void* gu, int M, int I, void* h, cudaStream_t st);
 

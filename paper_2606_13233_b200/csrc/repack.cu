@@ -1,7 +1,12 @@
 // repack.cu -- offline weight repack (step a0) and its exact inverse.  Pure byte permutation:
-// canonical codes[N,K/2] + scales[N,K/16]  <->  blob of 4608-byte cells (nvfp4_common.cuh; the
-// K-part count of the layout is a function of (N, K) only).
+// canonical codes[N,K/2] + scales[N,K/16]  <->  blob = 128-byte versioned header + 4608-byte cells
+// (nvfp4_common.cuh; the K-part count KP of the layout is recorded in the header).
 // Padding rows (n >= N) and padding k (k >= K) are zero codes / zero scales.
+//
+// Both launches end with an empty, ordinary (non-PDL) kernel: the GEMV is launched with programmatic
+// stream serialization and starts reading the blob BEFORE its griddepcontrol.wait, so its stream
+// predecessor must never be the kernel that writes the blob.  With the empty kernel in between, the
+// GEMV's predecessor starts only after the repack has completed and flushed.
 #include "nvfp4_common.cuh"
 #include "nvfp4_internal.h"
 
@@ -15,11 +20,16 @@ __global__ void __launch_bounds__(256) repack_kernel(uint8_t* __restrict__ codes
     constexpr int EPC = CELL_VECS * 32 + 32;                // code vectors + scale groups per cell
     const int64_t nvec = ncells * EPC;
     const int64_t rowb = K / 2, rows = K / 16;
+    if (TO_BLOB && blockIdx.x == 0 && threadIdx.x < BLOB_HEADER_BYTES / 4) {          // versioned header
+        const uint4 w = blob_header_words(N, K, L.kp);
+        const uint32_t h[8] = {w.x, w.y, w.z, w.w, (uint32_t)CELL_BYTES, (uint32_t)L.ntiles, (uint32_t)L.ncells, 0u};
+        reinterpret_cast<uint32_t*>(blob)[threadIdx.x] = threadIdx.x < 8 ? h[threadIdx.x] : 0u;
+    }
     for (int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; v < nvec; v += (int64_t)gridDim.x * blockDim.x) {
         const int64_t cell = v / EPC;
         const int e = (int)(v - cell * EPC);
         const int tile = (int)(cell / L.ncells), ci = (int)(cell - (int64_t)tile * L.ncells);
-        uint8_t* cellp = blob + cell * CELL_BYTES;
+        uint8_t* cellp = blob + BLOB_HEADER_BYTES + cell * CELL_BYTES;
         const int lane = e & 31;
         const int n = tile * L.rpt + lane % L.rpt, part = lane / L.rpt;      // lane = part * rpt + row
         if (e < CELL_VECS * 32) {
@@ -52,17 +62,21 @@ static int repack_grid(const Layout& L) {
     return (int)g;
 }
 
-cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob, cudaStream_t st) {
-    const Layout L = make_layout(N, K, layout_kparts(N, K));
+__global__ void pdl_fence_kernel() {}
+
+cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, int K, int kp, void* blob, cudaStream_t st) {
+    const Layout L = make_layout(N, K, kp);
     repack_kernel<true><<<repack_grid(L), 256, 0, st>>>(const_cast<uint8_t*>(codes), const_cast<uint8_t*>(scales),
                                                         N, K, L, static_cast<uint8_t*>(blob));
+    pdl_fence_kernel<<<1, 32, 0, st>>>();
     return cudaGetLastError();
 }
 
-cudaError_t launch_unpack(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st) {
-    const Layout L = make_layout(N, K, layout_kparts(N, K));
+cudaError_t launch_unpack(const void* blob, int N, int K, int kp, uint8_t* codes, uint8_t* scales, cudaStream_t st) {
+    const Layout L = make_layout(N, K, kp);
     repack_kernel<false><<<repack_grid(L), 256, 0, st>>>(codes, scales, N, K, L,
                                                          static_cast<uint8_t*>(const_cast<void*>(blob)));
+    pdl_fence_kernel<<<1, 32, 0, st>>>();
     return cudaGetLastError();
 }
 

@@ -35,16 +35,16 @@ def test_binding_lists_every_symbol():
 
 
 def test_version_and_sizes(lib):
-    assert lib.nvfp4_version() == 1
+    assert lib.nvfp4_version() == 2
     lib.nvfp4_repacked_bytes.restype = ctypes.c_size_t
-    # exactly the information of the canonical pair when N % 32 == 0 and K % 128 == 0
+    # exactly the information of the canonical pair (+ the 128-byte versioned header) when N % 32 == 0 and K % 256 == 0
     for N, K in [(2048, 2048), (10240, 5120), (5120, 8192), (51200, 5120), (5120, 25600)]:
-        assert lib.nvfp4_repacked_bytes(N, K) == N * K // 2 + N * K // 16
+        assert lib.nvfp4_repacked_bytes(N, K) == 128 + N * K // 2 + N * K // 16
     # ragged shapes: whole 4608-byte cells, never less than the canonical information, bounded padding
     for N, K in [(33, 144), (100, 208), (1, 16), (1000, 2576)]:
         b = lib.nvfp4_repacked_bytes(N, K)
-        assert b % 4608 == 0 and b >= N * K * 9 // 16
-        assert b <= (N + 31) * ((K + 255) // 256 * 256 * 1.04) * 9 / 16 + 4608
+        assert (b - 128) % 4608 == 0 and b - 128 >= N * K * 9 // 16
+        assert b - 128 <= (N + 31) * ((K + 255) // 256 * 256 * 1.04) * 9 / 16 + 4608
     assert lib.nvfp4_repacked_bytes(0, 128) == 0
     assert lib.nvfp4_repacked_bytes(32, 24) == 0          # K % 16 != 0
 
@@ -77,7 +77,12 @@ def test_config_table_is_sane(lib):
                 v = [ctypes.c_int(0) for _ in range(4)]
                 assert lib.nvfp4_gemv_get_config(mode, M, N, K, *[ctypes.byref(a) for a in v]) == 0
                 ks, warps, rows, stages = [a.value for a in v]
-                assert 1 <= ks <= (K + 255) // 256 and 1 <= warps <= 20 and rows in (1, 2, 4) and 1 <= stages <= 16
+                assert 1 <= ks <= (K + 255) // 256 and 1 <= warps <= 20 and rows in (1, 2) and 1 <= stages <= 16
             assert lib.nvfp4_gemv_workspace_bytes(M, N, K) > 0
     assert lib.nvfp4_gemv_set_config(0, 0, 3, 0) == -1
+    assert lib.nvfp4_gemv_set_config(0, 0, 4, 0) == -1
+    assert lib.nvfp4_set_layout_kparts(3) == -1 and lib.nvfp4_set_layout_kparts(64) == -1
+    assert lib.nvfp4_set_layout_kparts(4) == 0 and lib.nvfp4_get_layout_kparts(5120, 5120) == 4
+    assert lib.nvfp4_set_layout_kparts(0) == 0 and lib.nvfp4_get_layout_kparts(5120, 25600) == 4
+    assert lib.nvfp4_get_layout_kparts(51200, 5120) == 1
     assert lib.nvfp4_gemv_set_config(0, 0, 0, 0) == 0
