@@ -170,7 +170,12 @@ int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int
  * Launch-shape override for sweeps (process-wide host state behind a mutex; 0 = use the tuned table):
  *   ksplit = number of K slices (grid.y, 1..64), warps = consumer warps per CTA (1..20),
  *   rows   = row tiles per warp step (1 or 2; 2 exists for the integer W4A4 path, M >= 2),
- *   stages = depth of each warp's bulk-copy ring (1..16).
+ *   stages = depth of each warp's bulk-copy ring (1..16),
+ *   ctas_per_sm = persistent CTAs per SM (1..3; with >= 2 the CTAs of the NEXT kernel on the stream become
+ *            resident and prefetch their first weight cells while this kernel still runs),
+ *   balance = 1: every CTA owns units/CTAs whole row-tile units plus an equal share of the leftover units'
+ *            cells (data-parallel + stream-K, equal bytes per SM); 2: whole units only (the first CTAs own one
+ *            unit more; no partial sums between CTAs).
  * Values the kernels cannot run (shared memory, launch bounds) are clamped; nvfp4_gemv_get_config reports
  * what nvfp4_gemv would use for (mode, M, N, K).  Returns NVFP4_ERR_INVALID_ARG if out of range.
  * nvfp4_set_layout_kparts overrides the K-part count KP of the repacked layout (0 = the default function
@@ -178,8 +183,9 @@ int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int
  * process; the header records KP, so a blob repacked under another value is rejected (NaN outputs), never
  * misread.  nvfp4_get_layout_kparts returns the KP in effect for (N, K).
  */
-int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages);
-int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages);
+int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages, int ctas_per_sm, int balance);
+int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages,
+                          int* ctas_per_sm, int* balance);
 int nvfp4_set_layout_kparts(int kparts);
 int nvfp4_get_layout_kparts(int N, int K);
 

@@ -66,9 +66,9 @@ def _load():
     lib.nvfp4_gemv_fused_quant.restype = c_int
     lib.nvfp4_gemv_fused_quant.argtypes = [vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_set_config.restype = c_int
-    lib.nvfp4_gemv_set_config.argtypes = [c_int, c_int, c_int, c_int]
+    lib.nvfp4_gemv_set_config.argtypes = [c_int, c_int, c_int, c_int, c_int, c_int]
     lib.nvfp4_gemv_get_config.restype = c_int
-    lib.nvfp4_gemv_get_config.argtypes = [c_int, c_int, c_int, c_int] + [ctypes.POINTER(c_int)] * 4
+    lib.nvfp4_gemv_get_config.argtypes = [c_int, c_int, c_int, c_int] + [ctypes.POINTER(c_int)] * 6
     lib.nvfp4_silu_mul.restype = c_int
     lib.nvfp4_silu_mul.argtypes = [vp, c_int, c_int, vp, vp]
     return lib
@@ -177,14 +177,14 @@ def nvfp4_gemv_fused_quant(w_blob, w_gscale, N, K, x_bf16, x_gscale_out=None, y=
     return y
 
 
-def nvfp4_gemv_set_config(ksplit=0, warps=0, rows=0, stages=0):
-    _check(lib.nvfp4_gemv_set_config(ksplit, warps, rows, stages))
+def nvfp4_gemv_set_config(ksplit=0, warps=0, rows=0, stages=0, ctas_per_sm=0, balance=0):
+    _check(lib.nvfp4_gemv_set_config(ksplit, warps, rows, stages, ctas_per_sm, balance))
 
 
 def nvfp4_gemv_get_config(mode, M, N, K):
-    v = [ctypes.c_int(0) for _ in range(4)]
+    v = [ctypes.c_int(0) for _ in range(6)]
     _check(lib.nvfp4_gemv_get_config(mode, M, N, K, *[ctypes.byref(a) for a in v]))
-    return dict(ksplit=v[0].value, warps=v[1].value, rows=v[2].value, stages=v[3].value)
+    return dict(ksplit=v[0].value, warps=v[1].value, rows=v[2].value, stages=v[3].value, ctas_per_sm=v[4].value, balance=v[5].value)
 
 
 def nvfp4_set_layout_kparts(kparts=0):

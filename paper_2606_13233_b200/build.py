@@ -19,6 +19,8 @@ SOURCES = ["api.cu", "quantize.cu", "repack.cu", "gemv.cu", "gemv_w4a4.cu", "gem
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]        # NOTE: never -use_fast_math (bit-exact quantizer)
+if os.environ.get("NVFP4_ENABLE_TRACE"):                 # debug builds: %globaltimer stamps in the GEMV (nvfp4_debug_set_trace)
+    FLAGS.append("-DNVFP4_ENABLE_TRACE")
 
 
 def _deps():

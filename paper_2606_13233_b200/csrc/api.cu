@@ -10,11 +10,13 @@
 
 using namespace nvfp4;
 
+namespace nvfp4 { extern unsigned long long* g_trace; }
+
 static thread_local char g_last_err[256] = "";
 // process-wide knobs for sweeps (nvfp4_gemv_set_config, nvfp4_set_layout_kparts); 0 = use the tuned table.
 // Guarded by a mutex: a call reads one consistent snapshot.
 static std::mutex g_knob_mutex;
-static GemvConfig g_override = {0, 0, 0, 0};
+static GemvConfig g_override = {0, 0, 0, 0, -1, 0};    // whole: -1 = table
 static int g_kparts = 0;
 static GemvConfig override_snapshot(int* kp_out) {
     std::lock_guard<std::mutex> lock(g_knob_mutex);
@@ -43,6 +45,8 @@ static GemvConfig effective_config(int mode, int M, int N, int K, int kp) {
     if (o.warps > 0) c.warps = o.warps;
     if (o.rows > 0) c.rows = o.rows;
     if (o.stages > 0) c.stages = o.stages;
+    if (o.cps > 0) c.cps = o.cps;
+    if (o.whole >= 0) c.whole = o.whole;
     return gemv_legalize_config(mode, M, N, K, kp, c);
 }
 
@@ -155,11 +159,14 @@ int nvfp4_gemv_fused_quant(const void* w_blob, const float* w_gscale, int N, int
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
-int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages) {
+int nvfp4_gemv_set_config(int ksplit, int warps, int rows, int stages, int ctas_per_sm, int balance) {
     if (ksplit < 0 || ksplit > 64 || warps < 0 || warps > 20 || stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
+    if (ctas_per_sm < 0 || ctas_per_sm > 3 || balance < 0 || balance > 2) return NVFP4_ERR_INVALID_ARG;
     if (!(rows == 0 || rows == 1 || rows == 2)) return NVFP4_ERR_INVALID_ARG;
     std::lock_guard<std::mutex> lock(g_knob_mutex);
     g_override.ksplit = ksplit; g_override.warps = warps; g_override.rows = rows; g_override.stages = stages;
+    g_override.cps = ctas_per_sm;
+    g_override.whole = balance - 1;                 // 0 = table, 1 = data-parallel + stream-K, 2 = whole units only
     return NVFP4_OK;
 }
 
@@ -175,7 +182,7 @@ int nvfp4_get_layout_kparts(int N, int K) {
     return effective_kparts(N, K);
 }
 
-int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages) {
+int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps, int* rows, int* stages, int* ctas_per_sm, int* balance) {
     if (mode != NVFP4_MODE_W4A4 && mode != NVFP4_MODE_W4A16) return NVFP4_ERR_INVALID_ARG;
     if (!shape_ok(M, N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     const GemvConfig c = effective_config(mode, M, N, K, effective_kparts(N, K));
@@ -183,6 +190,15 @@ int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps
     if (warps) *warps = c.warps;
     if (rows) *rows = c.rows;
     if (stages) *stages = c.stages;
+    if (ctas_per_sm) *ctas_per_sm = c.cps;
+    if (balance) *balance = c.whole + 1;
+    return NVFP4_OK;
+}
+
+/* debug hook (not declared in include/nvfp4.h): device buffer of 16 x u64 per CTA that the GEMV fills with
+ * %globaltimer stamps of its phases; NULL switches tracing off. */
+int nvfp4_debug_set_trace(void* device_buffer) {
+    g_trace = static_cast<unsigned long long*>(device_buffer);
     return NVFP4_OK;
 }
 

@@ -5,12 +5,15 @@
 //  * lane <-> (weight row, K part): lane = p*(32/KP) + r.  The KP lanes of a row take interleaved 32-k
 //    vectors and are summed by log2(KP) warp shuffles once per segment.  KP is a property of the
 //    repacked layout (nvfp4_common.cuh).
-//  * STREAM-K: the weight of a K slice is one flat stream of `units * cells` 4608-byte cells (unit = R
-//    row tiles, cell = 256*KP k).  The stream is cut into gridDim.x EQUAL shares, one per CTA (about one
-//    CTA per SM), and every CTA's share into W equal shares, one per consumer warp: every SM and every
-//    warp streams the same number of bytes whatever N and K are.  A unit cut between warps is recombined
-//    through shared-memory slots, a unit cut between CTAs (or K slices) through FP32 partials in the
-//    workspace; both are summed in a fixed order by the last contributor to arrive -> deterministic.
+//  * BALANCE (data-parallel + stream-K): unit = R row tiles x all cells of the K slice (cell = 256*KP k,
+//    4608 B).  Every CTA (about one per SM) owns `base` = units / CTAs whole units (phase B) plus an EQUAL
+//    share of the flat cell stream of the leftover units (phase A), so every SM streams the same number of
+//    bytes whatever N and K are.  Phase A comes FIRST and its cells are dealt round-robin to the consumer
+//    warps (one cell each, typically), so the leftover units are finished within the first microseconds:
+//    their FP32 partials go through the workspace and the last CTA to arrive sums them in a fixed order
+//    (deterministic) -- on the otherwise idle stager warps, in the shadow of phase B.  Phase B is a
+//    contiguous run per warp; a unit cut between warps is recombined through shared-memory slots by the
+//    last warp to arrive, in fixed warp order.  With one K slice no CTA waits on another one at the end.
 //  * the activations of the CTA's K slice are decoded ONCE per CTA into shared memory by dedicated
 //    stager warps; lanes read them with LDS.128 (KP distinct addresses per instruction, conflict free).
 //  * each warp has a PRIVATE ring of S stages filled by 1-D bulk copies (cp.async.bulk ->
@@ -36,27 +39,35 @@ struct GemvParams {
     const uint8_t* x_scales;  // W4A4: [M, K/16]
     const float* x_gscale;    // W4A4: one float, or M floats (gscale_per_row)
     void* y;
-    float* partials;          // [ksplit][jmax][M][Npad]
+    float* partials_a;        // [ksplit][jmax][M][npad_a]: leftover units (phase A), one slot per contributing CTA
+    float* partials_b;        // [ksplit][M][npad_b]: whole units (phase B), used with K slices only
     unsigned int* counters;   // [units], zero on entry, zero on exit
     int64_t ldx, ldy;
-    int N, K, ntiles, nch, Npad;   // tiles of 32/kp rows, cells of 256*kp k, Npad = units * R * (32/kp)
+    int N, K, ntiles, nch;         // tiles of 32/kp rows, cells of 256*kp k
+    int npad_a, npad_b;            // padded row counts of the leftover / whole units
     int kp, kp_shift;              // K parts per row inside a warp (power of two) and its log2
     int warps, stages, ksplit;
     int units;                     // ceil(ntiles / R): a unit = R adjacent row tiles
     int cells_q, cells_r;          // nch / ksplit and nch % ksplit   (K slice `by` has q + (by < r) cells per unit)
-    // stream-K: slice variant v (0: cells_q cells per unit, 1: cells_q + 1) has T_v = units * cells flat cells;
-    // CTA b of gridDim.x owns [start_v(b), start_v(b+1)), start_v(b) = b*share_q[v] + (b*share_r[v]) / gridDim.x
-    int share_q[2], share_r[2];
-    float inv_share[2];            // gridDim.x / T_v (estimate for the inverse of start_v)
-    int jmax;                      // max number of CTAs of one slice that share a unit (partials slots)
-    int ucta_max;                  // max number of units a CTA touches
+    // work split: every CTA of a slice owns `base` whole units (phase B) and an equal
+    // share of the flat cell stream of the `ur` = units - base*gridDim.x leftover units (phase A).  Slice
+    // variant v (0: cells_q cells per unit, 1: cells_q + 1): nba[v] = min(gridDim.x, ur*ncw_v) CTAs take part
+    // in phase A; CTA b < nba owns leftover cells [b*a_q[v] + (b*a_r[v])/nba[v], same for b + 1).
+    int base, ur;
+    int whole_units;               // 1: no leftover stream; the first `ur` CTAs own base + 1 whole units instead
+    int nba[2], a_q[2], a_r[2];
+    float inv_a[2];                // nba / (ur*ncw_v): estimate for the inverse of the share start
+    int amax;                      // max leftover cells per CTA
+    int jmax;                      // max number of CTAs of one slice that share a leftover unit
     int nxb;                       // staging-batch mbarriers
+    int nhand;                     // hand-off slots: 2 leftover units (+ base whole units with K slices)
     int y_bf16;
     int zero;                      // always 0 (see make_wlut)
     int fuse_quant;                // x is BF16 [M,K] (ldx elements): quantise it inside the kernel (W4A4 modes)
     int gscale_per_row;            // x_gscale holds M per-row (per-token) global scales
     float* x_gscale_out;           // fuse_quant: optional device float that receives the activation global scale
     uint4 hdr_expect;              // blob_header_words(N, K, kp)
+    unsigned long long* trace;     // debug only (nvfp4_debug_set_trace): 16 timestamps per CTA, else NULL
 };
 
 // shared-memory bytes of activations per 32-k block pair and per m
@@ -113,17 +124,18 @@ __device__ __forceinline__ void decode_w_u8(const WLut& l, uint32_t w, uint32_t&
 }
 
 // ---- activation staging: decode the CTA's K range once into shared memory ----------------
-// Done by the CTA's dedicated STAGER warps (threads [W*32, W*32 + STAGER_THREADS)) while the
-// consumer warps already stream and multiply; readiness is signalled per batch through mbarriers.  Loads are issued STAGE_BATCH at a time per thread, so the L2
-// latency is paid once per batch.
-constexpr int STAGE_BATCH = 8;
+// Done by ALL threads of the CTA right after the consumer warps have requested their first weight cells (the
+// L2 round trip of the activation loads hides under the HBM latency of those cells); readiness is signalled
+// per batch through mbarriers.  Loads are issued STAGE_BATCH at a time per thread, so the L2 latency is paid
+// once per batch.  STAGER_WARPS extra warps take part in the staging and afterwards complete the row tiles
+// the CTA shares with other CTAs (closer role).
+constexpr int STAGE_BATCH = 4;
 constexpr int STAGER_WARPS = 4;
 constexpr int STAGER_THREADS = STAGER_WARPS * 32;
 
-// one mbarrier per staging batch (STAGER_THREADS * STAGE_BATCH work items): every stager thread
-// arrives on it after its stores (release), a consumer waits (acquire) on the batch that contains
-// the last item it needs -- no polling loop, no barrier among the stagers.
-constexpr int STAGE_ITEMS = STAGER_THREADS * STAGE_BATCH;
+// one mbarrier per staging batch (blockDim.x * STAGE_BATCH work items): every thread arrives on it
+// after its stores (release), a consumer waits (acquire) on the batch that contains the last item it
+// needs -- no polling loop, no CTA-wide barrier.
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
@@ -170,19 +182,19 @@ __device__ __forceinline__ void decode_x_block_h(uint2 cw, float sx, uint8_t* ba
 }
 
 template <int M, bool HALF>
-__device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
+__device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
                                              uint64_t* xbars) {
     const int nblk = ncw * 2 * CELL_VECS * p.kp;                 // 16-blocks in the range
     const int kb_total = p.K >> 4;
     const int kb0 = c0 * 2 * CELL_VECS * p.kp;
     const uint8_t* xc = static_cast<const uint8_t*>(p.x);
     const int total = nblk * M;
-    for (int base = 0; base < total; base += STAGER_THREADS * STAGE_BATCH) {
+    for (int base = 0, batch = 0; base < total; base += nthr * STAGE_BATCH, ++batch) {
         uint2 cw[STAGE_BATCH];
         uint32_t sb[STAGE_BATCH];
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = base + t * STAGER_THREADS + tid;
+            const int i = base + t * nthr + tid;
             const int blk = i / M, m = i - blk * M;
             cw[t] = make_uint2(0u, 0u);
             sb[t] = 0;
@@ -193,14 +205,14 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
         }
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = base + t * STAGER_THREADS + tid;
+            const int i = base + t * nthr + tid;
             if (i < total) {
                 const int blk = i / M, m = i - blk * M;
                 if (HALF) decode_x_block_h(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_H, M) + m * XBP_W4A4H, blk & 1);
                 else      decode_x_block(cw[t], e4m3_to_float((uint8_t)sb[t]), xs + (size_t)(blk >> 1) * xvec_stride(KMODE_W4A4_I8, M) + m * XBP_W4A4, blk & 1);
             }
         }
-        mbar_arrive(smem_u32(xbars + base / STAGE_ITEMS));
+        mbar_arrive(smem_u32(xbars + batch));
     }
 }
 
@@ -275,17 +287,17 @@ __device__ __forceinline__ void stage_x_fused(const GemvParams& p, uint8_t* xs, 
 
 // W4A16: work item i -> (8-element vector = i / M, m = i % M); progress published in 16-blocks
 template <int M>
-__device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid,
+__device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
                                               uint64_t* xbars) {
     const int nvec = ncw * 4 * CELL_VECS * p.kp;                 // 8-element vectors per row in the range
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
     const int total = nvec * M;
     const int k_base = c0 * 32 * CELL_VECS * p.kp;
-    for (int base = 0; base < total; base += STAGER_THREADS * STAGE_BATCH) {
+    for (int base = 0, batch = 0; base < total; base += nthr * STAGE_BATCH, ++batch) {
         uint4 raw[STAGE_BATCH];
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = base + t * STAGER_THREADS + tid;
+            const int i = base + t * nthr + tid;
             const int v = i / M, m = i - v * M;
             raw[t] = make_uint4(0, 0, 0, 0);
             if (i < total && k_base + v * 8 < p.K)
@@ -293,7 +305,7 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
         }
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
-            const int i = base + t * STAGER_THREADS + tid;
+            const int i = base + t * nthr + tid;
             if (i < total) {
                 const int v = i / M, m = i - v * M;
                 float* dst = reinterpret_cast<float*>(xs + (size_t)(v >> 2) * xvec_stride(KMODE_W4A16, M) + m * XBP_W4A16) + (v & 3) * 8;
@@ -307,7 +319,7 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
                 reinterpret_cast<float4*>(dst)[1] = hi;
             }
         }
-        mbar_arrive(smem_u32(xbars + base / STAGE_ITEMS));
+        mbar_arrive(smem_u32(xbars + batch));
     }
 }
 
@@ -403,8 +415,8 @@ __device__ __forceinline__ float h2_sum_f32(uint32_t h2) {
     return r;
 }
 template <int M, int R>
-__device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const uint8_t* xbp, const float (&sw)[R][8],
-                                                  int j, float (&acc)[R][M]) {
+__device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const uint8_t* xbp, const uint64_t (&swp)[R][4],
+                                                  int j, uint64_t (&accp)[R][M]) {
     uint32_t wh[R][16];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -418,7 +430,8 @@ __device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const ui
     for (int m = 0; m < M; ++m) {
         const uint4* xr = reinterpret_cast<const uint4*>(xbp + m * XBP_W4A4H);
         const uint4 x0 = xr[0], x1 = xr[1], x2 = xr[2], x3 = xr[3];
-        const float2 sx = *reinterpret_cast<const float2*>(xbp + m * XBP_W4A4H + 64);
+        const uint2 sxb = *reinterpret_cast<const uint2*>(xbp + m * XBP_W4A4H + 64);
+        const uint64_t sx2 = pack2u(sxb.x, sxb.y);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             // two independent 4-deep chains per block, merged by an exact HADD2 (|sums| <= 288)
@@ -431,9 +444,10 @@ __device__ __forceinline__ void block_pair_w4a4_h(const uint4 (&wv)[R], const ui
             a0 = hfma2(wh[r][3], x0.w, a0); b0 = hfma2(wh[r][7], x1.w, b0);
             a1 = hfma2(wh[r][11], x2.w, a1); b1 = hfma2(wh[r][15], x3.w, b1);
             a0 = hadd2(a0, b0); a1 = hadd2(a1, b1);
-            const float p0 = sw[r][2 * j] * sx.x, p1 = sw[r][2 * j + 1] * sx.y;
-            acc[r][m] = fmaf(h2_sum_f32(a0), p0, acc[r][m]);    // f32(lo) + f32(hi): exact (|sum| <= 576)
-            acc[r][m] = fmaf(h2_sum_f32(a1), p1, acc[r][m]);
+            // f32(lo) + f32(hi) per block: exact (|sum| <= 576); the two blocks' sW*sX products and the
+            // accumulation ride in packed FP32 (one FMUL2 + one FFMA2 per row, m and block pair)
+            const uint64_t dots = pack2u(__float_as_uint(h2_sum_f32(a0)), __float_as_uint(h2_sum_f32(a1)));
+            accp[r][m] = ffma2_i8(dots, fmul2(swp[r][j], sx2), accp[r][m]);
         }
     }
 }
@@ -487,174 +501,201 @@ __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uin
 }
 
 // ---- shared-memory carve-up: ONE definition for the host (gemv_smem_bytes) and the kernel -----------
-struct SmemMap { uint32_t xs, ring, slots, bars, xbars, cnt, fstart, cstart, misc, total; };
+struct SmemMap { uint32_t xs, ring, slots, aslots, hand, bars, xbars, hbars, cnt, bstart, astart, misc, total; };
 __host__ __device__ inline SmemMap gemv_smem_map(int kmode, int M, int R, int W, int S, int rpt, int ncw_max, int kp,
-                                                 int nxb, int ucta_max, int nb) {
+                                                 int nxb, int base, int nb, int amax, int nhand) {
     SmemMap m;
     uint32_t o = 0;
+    const uint32_t slot_bytes = (uint32_t)R * M * rpt * 4;
     m.xs = o;     o += ((uint32_t)ncw_max * CELL_VECS * kp * xvec_stride(kmode, M) + 127u) & ~127u;   // activation records
     m.ring = o;   o += (uint32_t)W * S * R * CELL_BYTES;                   // per-warp bulk-copy rings
-    m.slots = o;  o += (uint32_t)W * 2 * R * M * rpt * 4;                  // segment partials (two per warp)
+    m.slots = o;  o += (uint32_t)W * 2 * slot_bytes;                       // phase B segment partials (two per warp)
+    m.aslots = o; o += (uint32_t)amax * slot_bytes;                        // phase A: one partial per leftover cell
+    m.hand = o;   o += (uint32_t)nhand * slot_bytes;                       // CTA sums handed to the closer warps
+    o = (o + 7u) & ~7u;
     m.bars = o;   o += (uint32_t)W * S * 8;                                // ring mbarriers
     m.xbars = o;  o += (uint32_t)nxb * 8;                                  // staging-batch mbarriers
-    m.cnt = o;    o += (uint32_t)ucta_max * 4;                             // per-unit arrival counters (warps)
-    m.fstart = o; o += (uint32_t)(W + 1) * 4;                              // warp share starts
-    m.cstart = o; o += (uint32_t)2 * (nb + 1) * 4;                         // CTA share starts, both slice variants
-    m.misc = o;   o += (2 + 32) * 4;                                       // fused quantizer: gX slot + per-warp amax
+    m.hbars = o;  o += (uint32_t)nhand * 8;                                // hand-off mbarriers
+    m.cnt = o;    o += (uint32_t)(base + 3) * 4;                           // arrival counters: [0,1] leftover units, [2..] whole units
+    m.bstart = o; o += (uint32_t)(W + 1) * 4;                              // phase B: warp share starts
+    m.astart = o; o += (uint32_t)2 * (nb + 1) * 4;                         // phase A: CTA share starts, both slice variants
+    m.misc = o;   o += (2 + 32) * 4;                                       // [0] fused gX, [1] blob-ok flag, [2..] per-warp amax
     m.total = (o + 15u) & ~15u;
     return m;
 }
 
-// CTA-constant context of the stream-K bookkeeping
+// CTA-constant context of the work split
 struct CtaCtx {
     int ncw;            // cells per unit in this CTA's K slice
-    int o, L;           // the CTA's share in local coordinates: cells [o, o + L), unit boundaries at multiples of ncw
-    int ub;             // global index of local unit 0
     int var;            // slice variant (0: cells_q, 1: cells_q + 1 cells per unit)
     int nb;             // CTAs per slice
-    const int* cstart;  // [2][nb + 1] share starts per variant
+    int unit0;          // phase B: global index of this CTA's first whole unit
+    int a0, na;         // phase A: this CTA's leftover cells [a0, a0 + na) of the slice's leftover stream
+    int qa0, n0;        // first leftover unit touched, and how many of the na cells belong to it
+    const int* astart;  // [2][nb + 1] leftover share starts per variant (entries above nba repeat the end)
 };
 
-// CTAs of a variant-v slice whose share intersects unit `unit`: [lo, hi].  start_v(b) is non-decreasing
-// with start_v(0) = 0; the float estimate is corrected against the table.
-__device__ __forceinline__ void contrib_range(const GemvParams& p, const CtaCtx& c, int v, int unit, int& lo, int& hi) {
-    const int ncw_v = p.cells_q + v;
-    const int* cs = c.cstart + v * (c.nb + 1);
-    const int x0 = unit * ncw_v, x1 = x0 + ncw_v - 1;
-    int b = (int)((float)x0 * p.inv_share[v]);
-    b = b < 0 ? 0 : (b > c.nb - 1 ? c.nb - 1 : b);
-    while (b + 1 < c.nb && cs[b + 1] <= x0) ++b;
+// CTAs of a variant-v slice whose leftover share intersects leftover unit q: [lo, hi].  The starts are
+// strictly increasing over the nba participating CTAs; the float estimate is corrected against the table.
+__device__ __forceinline__ void contrib_range(const GemvParams& p, const CtaCtx& c, int v, int q, int& lo, int& hi) {
+    const int ncw_v = p.cells_q + v, nba = p.nba[v];
+    const int* cs = c.astart + v * (c.nb + 1);
+    const int x0 = q * ncw_v, x1 = x0 + ncw_v - 1;
+    int b = (int)((float)x0 * p.inv_a[v]);
+    b = b < 0 ? 0 : (b > nba - 1 ? nba - 1 : b);
+    while (b + 1 < nba && cs[b + 1] <= x0) ++b;
     while (cs[b] > x0) --b;
     lo = b;
-    while (b + 1 < c.nb && cs[b + 1] <= x1) ++b;
+    while (b + 1 < nba && cs[b + 1] <= x1) ++b;
     hi = b;
 }
 
-// ---- a7: write one finished unit (R tiles); `acc` holds the CTA's complete sums for the unit over its
-// cells in the writer lanes (part == 0).  If the CTA does not hold the unit's whole K range (the stream-K cut
-// fell inside the unit, or K is sliced across grid.y) the FP32 partial goes to the workspace and the last
-// CTA to arrive for this unit sums all contributions in a fixed order (slice-major, then CTA order).
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#ifdef NVFP4_ENABLE_TRACE      // debug builds only (-DNVFP4_ENABLE_TRACE): per-phase %globaltimer stamps, 64 per CTA
+#define NVFP4_TRACE(slot) do { if (p.trace) p.trace[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 64 + (slot)] = globaltimer_ns(); } while (0)
+#else
+#define NVFP4_TRACE(slot) do { } while (0)
+#endif
+
+__device__ __forceinline__ void store_y(const GemvParams& p, int m, int n, float v) {
+    if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
+    else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
+}
+
+// ---- a7 (closer warps): complete a unit this CTA holds only a part of.  `hand` = the CTA's FP32 sums
+// [(r*M + m)*rpt + row].  kind A: leftover unit q (cut between CTAs, and between K slices); kind B: whole unit
+// (cut between K slices only).  The partial goes to the workspace; the last CTA to arrive for the unit sums all
+// contributions in a fixed order (slice-major, then CTA order) and writes the outputs.
 template <int M, int R>
-__device__ __forceinline__ void emit_unit(const GemvParams& p, const CtaCtx& c, float (&acc)[R][M], int ul, int lane,
-                                          bool writer, int rsub, int rpt, float gs) {
-    const int unit = c.ub + ul;
-    int nvalid = p.ntiles - unit * R;
-    nvalid = nvalid > R ? R : nvalid;
-    const bool cta_whole = (p.ksplit == 1) && (ul * c.ncw >= c.o) && ((ul + 1) * c.ncw <= c.o + c.L);
-    if (!cta_whole) {
-        int lo0 = 0, hi0 = -1, lo1 = 0, hi1 = -1;
-        const int nvar1 = p.cells_r, nvar0 = p.ksplit - p.cells_r;          // slices per variant
-        if (nvar0 > 0) contrib_range(p, c, 0, unit, lo0, hi0);
-        if (nvar1 > 0) contrib_range(p, c, 1, unit, lo1, hi1);
-        const int myslot = (int)blockIdx.y * p.jmax + ((int)blockIdx.x - (c.var ? lo1 : lo0));
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int n = (unit * R + r) * rpt + rsub;
-            if (writer && r < nvalid) {
-#pragma unroll
-                for (int m = 0; m < M; ++m)
-                    __stcg(p.partials + ((int64_t)myslot * M + m) * p.Npad + n, acc[r][m]);
-            }
-        }
-        __threadfence();
-        __syncwarp();
-        unsigned int last = 0;
-        if (lane == 0) {
-            const unsigned int expected = (unsigned int)(nvar0 * (hi0 - lo0 + 1) + nvar1 * (hi1 - lo1 + 1));
-            const unsigned int old = atomicAdd(p.counters + unit, 1u);
-            last = (old == expected - 1u);
-            if (last) p.counters[unit] = 0u;                              // leave the workspace clean
-        }
-        last = __shfl_sync(0xFFFFFFFFu, last, 0);
-        if (!last) return;
-        __threadfence();
-#pragma unroll
-        for (int r = 0; r < R; ++r)
-#pragma unroll
-            for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
-        for (int ks = 0; ks < p.ksplit; ++ks) {
-            const int nj = ks < p.cells_r ? (hi1 - lo1) : (hi0 - lo0);
-            for (int j = 0; j <= nj; ++j) {
-                const float* src = p.partials + (int64_t)(ks * p.jmax + j) * M * p.Npad;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const int n = (unit * R + r) * rpt + rsub;
-                    if (writer && r < nvalid) {
-#pragma unroll
-                        for (int m = 0; m < M; ++m) acc[r][m] += __ldcg(src + (int64_t)m * p.Npad + n);
-                    }
-                }
-            }
-        }
+__device__ __forceinline__ void close_unit(const GemvParams& p, const CtaCtx& c, const float* hand, bool kind_a, int idx,
+                                           int lane, int rpt, float gs) {
+    // idx: kind A -> leftover unit q; kind B -> local whole unit ul
+    const int unit = kind_a ? (p.base * c.nb + idx) : (c.unit0 + idx);
+    const int prow0 = (kind_a ? idx : unit) * R * rpt;                  // first row inside partials_a / partials_b
+    int lo0 = 0, hi0 = -1, lo1 = 0, hi1 = -1;
+    const int nvar1 = p.cells_r, nvar0 = p.ksplit - p.cells_r;          // slices per variant
+    unsigned int expected = (unsigned int)p.ksplit;
+    float* mine;
+    if (kind_a) {
+        if (nvar0 > 0) contrib_range(p, c, 0, idx, lo0, hi0);
+        if (nvar1 > 0) contrib_range(p, c, 1, idx, lo1, hi1);
+        expected = (unsigned int)(nvar0 * (hi0 - lo0 + 1) + nvar1 * (hi1 - lo1 + 1));
+        mine = p.partials_a + (int64_t)((int)blockIdx.y * p.jmax + ((int)blockIdx.x - (c.var ? lo1 : lo0))) * M * p.npad_a;
+    } else {
+        mine = p.partials_b + (int64_t)blockIdx.y * M * p.npad_b;
     }
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int n = (unit * R + r) * rpt + rsub;
-        if (writer && r < nvalid && n < p.N) {
-#pragma unroll
-            for (int m = 0; m < M; ++m) {
-                // per-token activation scales (nvfp4_gemv_rowscale): gs holds the weight-side factor only
-                const float v = acc[r][m] * (p.gscale_per_row ? gs * __ldg(p.x_gscale + m) : gs);
-                if (p.y_bf16) static_cast<uint16_t*>(p.y)[(int64_t)m * p.ldy + n] = float_to_bf16_rn(v);
-                else          static_cast<float*>(p.y)[(int64_t)m * p.ldy + n] = v;
+    const int npad = kind_a ? p.npad_a : p.npad_b;
+    const int nval = R * M * rpt;
+    for (int i = lane; i < nval; i += 32) {
+        const int row = i % rpt, rm = i / rpt, m = rm % M, r = rm / M;
+        __stcg(mine + (int64_t)m * npad + prow0 + r * rpt + row, hand[i]);
+    }
+    __threadfence();
+    __syncwarp();
+    unsigned int last = 0;
+    if (lane == 0) {
+        const unsigned int old = atomicAdd(p.counters + unit, 1u);
+        last = (old == expected - 1u);
+        if (last) p.counters[unit] = 0u;                              // leave the workspace clean
+    }
+    last = __shfl_sync(0xFFFFFFFFu, last, 0);
+    if (!last) return;
+    __threadfence();
+    for (int i = lane; i < nval; i += 32) {
+        const int row = i % rpt, rm = i / rpt, m = rm % M, r = rm / M;
+        const int n = (unit * R + r) * rpt + row;
+        if (unit * R + r >= p.ntiles || n >= p.N) continue;
+        float sum = 0.0f;
+        for (int ks = 0; ks < p.ksplit; ++ks) {
+            if (kind_a) {
+                const int nj = ks < p.cells_r ? (hi1 - lo1) : (hi0 - lo0);
+                for (int j = 0; j <= nj; ++j)
+                    sum += __ldcg(p.partials_a + ((int64_t)(ks * p.jmax + j) * M + m) * npad + prow0 + r * rpt + row);
+            } else {
+                sum += __ldcg(p.partials_b + ((int64_t)ks * M + m) * npad + prow0 + r * rpt + row);
             }
         }
+        store_y(p, m, n, sum * (p.gscale_per_row ? gs * __ldg(p.x_gscale + m) : gs));
     }
 }
 
-// first cell of consumer warp w's share of the CTA's L cells (W <= L <= 2^26)
-__device__ __forceinline__ int flat_start(int w, int L, int W) { return (int)(((unsigned)w * (unsigned)L) / (unsigned)W); }
-
-// ---- a6: a warp finished its segment of local unit `ul`.  K parts of a row are summed by shuffles; a
-// unit shared by several warps is combined through shared-memory slots (two per warp: slot 0 = the
-// segment that starts the warp's share, slot 1 = any later one) by the LAST warp to arrive, in fixed
-// warp order -> deterministic.
+// K parts of a row are summed by shuffles (lanes of one row are rpt apart)
 template <int M, int R>
-__device__ __forceinline__ void finish_segment(const GemvParams& p, const CtaCtx& c, float (&acc)[R][M], float* slots,
-                                               int* cnt, const int* fstart, int ul, bool whole, bool seg_at_share_start,
-                                               int warp, int lane, int part, int rsub, int rpt, float gs) {
-    for (int off = rpt; off < 32; off <<= 1) {                  // lanes of one row are rpt apart
+__device__ __forceinline__ void reduce_parts(float (&acc)[R][M], int rpt) {
+    for (int off = rpt; off < 32; off <<= 1) {
 #pragma unroll
         for (int r = 0; r < R; ++r)
 #pragma unroll
             for (int m = 0; m < M; ++m) acc[r][m] += __shfl_xor_sync(0xFFFFFFFFu, acc[r][m], off);
     }
+}
+// the CTA's sums of a finished unit: outputs (the CTA holds the whole unit) or hand-off to a closer warp
+template <int M, int R>
+__device__ __forceinline__ void emit_or_hand(const GemvParams& p, float (&acc)[R][M], bool direct, int unit, float* hand,
+                                             uint64_t* hbars, int h, int lane, bool writer, int rsub, int rpt, float gs) {
+    if (direct) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int n = (unit * R + r) * rpt + rsub;
+            if (writer && unit * R + r < p.ntiles && n < p.N) {
+#pragma unroll
+                for (int m = 0; m < M; ++m)
+                    store_y(p, m, n, acc[r][m] * (p.gscale_per_row ? gs * __ldg(p.x_gscale + m) : gs));
+            }
+        }
+    } else {
+        float* dst = hand + (size_t)h * (R * M * rpt);
+        if (writer) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int m = 0; m < M; ++m) dst[(r * M + m) * rpt + rsub] = acc[r][m];
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(hbars + h));
+    }
+}
+__device__ __forceinline__ int arrive_count(int* cnt_word, int lane) {     // CTA-scope acq_rel arrival; old value to all lanes
+    int old = 0;
+    __syncwarp();                                   // the writer lanes' slot stores are ordered before the arrival
+    if (lane == 0)
+        asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(cnt_word)) : "memory");
+    return __shfl_sync(0xFFFFFFFFu, old, 0);
+}
+
+// ---- a6, phase A: a warp finished leftover cell i (0 <= i < na) of this CTA.  Every leftover cell is its own
+// segment; its partial goes to aslots[i]; the last cell of a leftover unit to arrive sums the unit's cells in
+// index order (deterministic) and hands the CTA's sum to a closer warp (or writes it, if the CTA holds the
+// whole unit and K is not sliced).
+template <int M, int R>
+__device__ __forceinline__ void finish_leftover_cell(const GemvParams& p, const CtaCtx& c, float (&acc)[R][M], float* aslots,
+                                                     float* hand, uint64_t* hbars, int* cnt, int i, int lane, int part,
+                                                     int rsub, int rpt, float gs) {
+    reduce_parts<M, R>(acc, rpt);
     const bool writer = (part == 0);
-    if (!whole) {
-        const int W = p.warps;
-        const int slot_floats = R * M * rpt;
-        float* mine = slots + (size_t)(warp * 2 + (seg_at_share_start ? 0 : 1)) * slot_floats;
+    const int slot_floats = R * M * rpt;
+    const int qa = i < c.n0 ? 0 : 1;                                         // which of the (at most two) leftover units
+    const int ilo = qa ? c.n0 : 0, ihi = qa ? c.na - 1 : c.n0 - 1;
+    if (ihi > ilo) {
+        float* mine = aslots + (size_t)i * slot_floats;
         if (writer) {
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int m = 0; m < M; ++m) mine[(r * M + m) * rpt + rsub] = acc[r][m];
         }
-        // contributors of this unit: warps whose share intersects [ul*ncw, (ul+1)*ncw)  (fstart[0] = o, so a
-        // unit that begins before the CTA's share starts at warp 0; one that ends after it ends at warp W-1)
-        const int lo = ul * c.ncw, hi = lo + c.ncw - 1;
-        int w_first = 0, w_last = 0;
-        for (int w = 0; w < W; ++w) {
-            const int fs = fstart[w];
-            if (fs <= lo) w_first = w;
-            if (fs <= hi) w_last = w;
-        }
-        __syncwarp();                                   // the writer lanes' slot stores are ordered before ...
-        int last = 0;
-        if (lane == 0) {                                // ... this CTA-scope acq_rel arrival (no separate fences)
-            int old;
-            asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(cnt + ul)) : "memory");
-            last = (old == w_last - w_first);
-        }
-        last = __shfl_sync(0xFFFFFFFFu, last, 0);
-        if (!last) return;
+        if (arrive_count(cnt + qa, lane) != ihi - ilo) return;
         if (writer) {
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
-            for (int w = w_first; w <= w_last; ++w) {
-                const float* sl = slots + (size_t)(w * 2 + (fstart[w] >= lo ? 0 : 1)) * slot_floats;
+            for (int k = ilo; k <= ihi; ++k) {
+                const float* sl = aslots + (size_t)k * slot_floats;
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -662,18 +703,68 @@ __device__ __forceinline__ void finish_segment(const GemvParams& p, const CtaCtx
             }
         }
     }
-    emit_unit<M, R>(p, c, acc, ul, lane, writer, rsub, rpt, gs);
+    const bool direct = (p.ksplit == 1) && (ihi - ilo + 1 == c.ncw);
+    emit_or_hand<M, R>(p, acc, direct, p.base * c.nb + c.qa0 + qa, hand, hbars, qa, lane, writer, rsub, rpt, gs);
 }
 
-// threads per CTA the instantiation is compiled for (consumer + stager warps)
+// ---- a6, phase B: a warp finished its segment of local whole unit `ul`.  A unit shared by several warps is
+// combined through shared-memory slots (two per warp: slot 0 = the segment that starts the warp's run,
+// slot 1 = its last one; every other segment covers a whole unit) by the LAST warp to arrive, in fixed warp
+// order -> deterministic.
+template <int M, int R>
+__device__ __forceinline__ void finish_segment(const GemvParams& p, const CtaCtx& c, float (&acc)[R][M], float* slots,
+                                               float* hand, uint64_t* hbars, int* cnt, const int* bstart, int ul,
+                                               bool whole, bool seg_at_run_start, int warp, int lane, int part, int rsub,
+                                               int rpt, float gs) {
+    reduce_parts<M, R>(acc, rpt);
+    const bool writer = (part == 0);
+    const int slot_floats = R * M * rpt;
+    if (!whole) {
+        const int W = p.warps;
+        float* mine = slots + (size_t)(warp * 2 + (seg_at_run_start ? 0 : 1)) * slot_floats;
+        if (writer) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int m = 0; m < M; ++m) mine[(r * M + m) * rpt + rsub] = acc[r][m];
+        }
+        // contributors of this unit: warps whose run intersects [ul*ncw, (ul+1)*ncw) (every warp has >= 1 cell)
+        const int lo = ul * c.ncw, hi = lo + c.ncw - 1;
+        int w_first = 0, w_last = 0;
+        for (int w = 0; w < W; ++w) {
+            const int fs = bstart[w];
+            if (fs <= lo) w_first = w;
+            if (fs <= hi) w_last = w;
+        }
+        if (arrive_count(cnt + 2 + ul, lane) != w_last - w_first) return;
+        if (writer) {
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
+            for (int w = w_first; w <= w_last; ++w) {
+                const float* sl = slots + (size_t)(w * 2 + (bstart[w] >= lo ? 0 : 1)) * slot_floats;
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+#pragma unroll
+                    for (int m = 0; m < M; ++m) acc[r][m] += *(volatile const float*)(sl + (r * M + m) * rpt + rsub);
+            }
+        }
+    }
+    emit_or_hand<M, R>(p, acc, p.ksplit == 1, c.unit0 + ul, hand, hbars, 2 + ul, lane, writer, rsub, rpt, gs);
+}
+
+// threads per CTA the instantiation is compiled for (consumer + stager warps): the FP16 path (M = 1) runs up to
+// 16 consumer warps at <= 102 registers; the integer and W4A16 paths 12 consumer warps at 128 registers (no
+// spills in the main loop: profiles/r02_ptxas.md; 12 warps measured as fast as 16 at M >= 2)
 __host__ __device__ constexpr int gemv_max_threads(int kmode, int M, int R) {
-    if (kmode == KMODE_W4A4_H && M == 1 && R == 1) return 768;
-    if (R >= 2) return 512;                               // 12 consumer warps, 128 registers
-    if (kmode == KMODE_W4A4_I8 && M >= 7) return 512;     // 128 registers: no spills at M = 7, 8
-    return 640;
+    if (kmode == KMODE_W4A4_H) return 640;
+    if (kmode == KMODE_W4A4_I8 && M <= 2 && R == 1) return 640;           // 16 consumer warps at <= 102 registers
+    return 512;
 }
 
-// Persistent, stream-K balanced (see the file header).  STAGER_WARPS extra warps decode the activations.
+// Persistent and balanced (see the file header).  STAGER_WARPS extra warps help to decode the activations and
+// afterwards complete the row tiles this CTA shares with other CTAs.
 template <int MODE, int M, int R>
 __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -681,9 +772,8 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const int W = p.warps, S = p.stages;
     const int rsub = lane & ((32 >> p.kp_shift) - 1), part = lane >> (5 - p.kp_shift);   // lane = part*rpt + rsub
     const int rpt = 32 >> p.kp_shift;
-    constexpr int XBP = xbp_bytes(MODE);
-    (void)XBP;
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
+    if (threadIdx.x == 0) NVFP4_TRACE(0);
 
     // K slice of this CTA (whole cells of 256*kp k); quotients and remainders come from the host
     const int by = blockIdx.y, bx = blockIdx.x, nb = gridDim.x;
@@ -694,75 +784,84 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const int ncw = p.cells_q + c.var;
     c.ncw = ncw;
     const int ncw_max = p.cells_q + (p.cells_r > 0 ? 1 : 0);
-    // this CTA's equal share [F0, F1) of the slice's flat stream of units * ncw cells
-    const unsigned F0 = (unsigned)bx * (unsigned)p.share_q[c.var] + ((unsigned)bx * (unsigned)p.share_r[c.var]) / (unsigned)nb;
-    const unsigned F1 = (unsigned)(bx + 1) * (unsigned)p.share_q[c.var] + ((unsigned)(bx + 1) * (unsigned)p.share_r[c.var]) / (unsigned)nb;
-    c.L = (int)(F1 - F0);
-    c.ub = (int)(F0 / (unsigned)ncw);
-    c.o = (int)(F0 - (unsigned)c.ub * (unsigned)ncw);
-    const int L = c.L;
+    // phase A: this CTA's equal share of the leftover units' flat cell stream; phase B: `base` whole units
+    {
+        const unsigned nba = (unsigned)p.nba[c.var], aq = (unsigned)p.a_q[c.var], ar = (unsigned)p.a_r[c.var];
+        unsigned a0 = 0, a1 = 0;
+        if ((unsigned)bx < nba) {
+            a0 = (unsigned)bx * aq + ((unsigned)bx * ar) / nba;
+            a1 = (unsigned)(bx + 1) * aq + ((unsigned)(bx + 1) * ar) / nba;
+        }
+        c.a0 = (int)a0; c.na = (int)(a1 - a0);
+        c.qa0 = (int)(a0 / (unsigned)ncw);
+        const int room = (c.qa0 + 1) * ncw - c.a0;                          // cells left in the first leftover unit
+        c.n0 = c.na < room ? c.na : room;
+    }
+    const int my_base = p.base + ((p.whole_units && bx < p.ur) ? 1 : 0);   // whole units of this CTA ...
+    c.unit0 = bx * p.base + (p.whole_units ? (bx < p.ur ? bx : p.ur) : 0);  // ... starting at this global unit
+    const int Bc = my_base * ncw;                                           // phase B cells of this CTA
 
-    const SmemMap map = gemv_smem_map(MODE, M, R, W, S, rpt, ncw_max, p.kp, p.nxb, p.ucta_max, nb);
+    const SmemMap map = gemv_smem_map(MODE, M, R, W, S, rpt, ncw_max, p.kp, p.nxb, p.base, nb, p.amax, p.nhand);
     uint8_t* xs = smem + map.xs;                                             // activations
     constexpr int XVS = xvec_stride(MODE, M);
     uint8_t* ring_all = smem + map.ring;
     float* slots = reinterpret_cast<float*>(smem + map.slots);
+    float* aslots = reinterpret_cast<float*>(smem + map.aslots);
+    float* hand = reinterpret_cast<float*>(smem + map.hand);
     uint64_t* bars_all = reinterpret_cast<uint64_t*>(smem + map.bars);
     uint64_t* xbars = reinterpret_cast<uint64_t*>(smem + map.xbars);
+    uint64_t* hbars = reinterpret_cast<uint64_t*>(smem + map.hbars);
     int* cnt = reinterpret_cast<int*>(smem + map.cnt);
-    int* fstart = reinterpret_cast<int*>(smem + map.fstart);
-    int* cstart = reinterpret_cast<int*>(smem + map.cstart);
+    int* bstart = reinterpret_cast<int*>(smem + map.bstart);
+    int* astart = reinterpret_cast<int*>(smem + map.astart);
     float* gx_slot = reinterpret_cast<float*>(smem + map.misc);
+    volatile int* blob_flag = reinterpret_cast<volatile int*>(smem + map.misc) + 1;
     uint32_t* red = reinterpret_cast<uint32_t*>(smem + map.misc) + 2;
-    c.cstart = cstart;
+    c.astart = astart;
     const bool fused = (MODE != KMODE_W4A16) && p.fuse_quant;
-    const int stage_items = fused ? (int)blockDim.x : STAGE_ITEMS;          // items per staging batch
+    const int stage_items = fused ? (int)blockDim.x : (int)blockDim.x * STAGE_BATCH;   // items per staging batch
 
-    for (int i = threadIdx.x; i < p.ucta_max; i += blockDim.x) cnt[i] = 0;
-    if (threadIdx.x <= W) fstart[threadIdx.x] = c.o + flat_start(threadIdx.x, L, W);
-    if (threadIdx.x <= nb) {                                                // blockDim.x >= 160 > nb
-        const unsigned b = threadIdx.x;
-        cstart[b] = (int)(b * (unsigned)p.share_q[0] + (b * (unsigned)p.share_r[0]) / (unsigned)nb);
-        cstart[nb + 1 + b] = (int)(b * (unsigned)p.share_q[1] + (b * (unsigned)p.share_r[1]) / (unsigned)nb);
-    }
-    for (int i = threadIdx.x; i < p.nxb; i += blockDim.x)
-        mbar_init(smem_u32(xbars + i), fused ? blockDim.x : STAGER_THREADS);
-    if (threadIdx.x == 0) mbar_fence_init();
-    __syncthreads();
-
-    if (warp >= W) {                                                        // ---- stager warps ----
-        const int tid = threadIdx.x - W * 32;
-        pdl_wait();                                   // the activations come from the previous kernel
-        if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, tid, xbars);
-        else if (p.fuse_quant)
-            stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
-        else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, tid, xbars);
-        return;
-    }
-
-    // ---- consumer warps ----
-    uint8_t* ring = ring_all + (size_t)warp * S * STAGE_BYTES;
-    uint64_t* bars = bars_all + warp * S;
-    const int f0 = fstart[warp], f1 = fstart[warp + 1];
-    const int f0_ul = (int)((unsigned)f0 / (unsigned)ncw);
-    const int total = f1 - f0;
+    // ---- consumer warps: request the first weight cells before anything else (private ring, private barriers) ----
+    // warp w: phase A cells i = w, w + W, ... < na (na_w of them), then phase B cells [bs, be) of the CTA's Bc
+    const bool consumer = warp < W;
+    const int na_w = consumer ? (c.na + W - 1 - warp) / W : 0;
+    const int bs = consumer ? Bc - (int)(((unsigned)(W - warp) * (unsigned)Bc) / (unsigned)W) : 0;
+    const int be = consumer ? Bc - (int)(((unsigned)(W - warp - 1) * (unsigned)Bc) / (unsigned)W) : 0;
+    const int total = na_w + (be - bs);
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
-
-    // producer cursor (used by lane 0 only): next cell to request.  Within a unit the cells of a
-    // tile are contiguous in the blob; with one K slice and R == 1 the whole share is one run.
-    const bool leader = (lane == 0);
-    int p_left = 0, p_count = 0, p_nv = 0;
+    uint8_t* ring = ring_all + (size_t)(consumer ? warp : 0) * S * STAGE_BYTES;
+    uint64_t* bars = bars_all + (consumer ? warp : 0) * S;
+    const bool leader = consumer && (lane == 0);
+    // producer cursor (used by lane 0 only): next cell to request.  The warp's cells form RUNS of cells that are
+    // contiguous in the blob: every leftover cell is a run of one, then one run per whole unit touched.
+    int p_left = 0, p_count = 0, p_nv = 0, p_a = 0;
+    bool p_b_started = false;
     uint32_t p_dst = smem_u32(ring), p_bar = smem_u32(bars);
     const uint32_t ring_end = p_dst + (uint32_t)S * STAGE_BYTES;
     const uint8_t* p_src = nullptr;
-    {
-        const int ul = f0_ul, cell = f0 - ul * ncw;
-        const int tile0 = (c.ub + ul) * R;
-        p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
-        p_left = ncw - cell;
-        p_nv = p.ntiles - tile0; p_nv = p_nv > R ? R : p_nv;
-    }
     const int64_t unit_jump = (int64_t)(R - 1) * tile_stride + (int64_t)(p.nch - ncw) * CELL_BYTES;
+    auto next_run = [&]() {
+        int tile0;
+        if (p_a < na_w) {                                                   // phase A: leftover cell i = warp + p_a*W
+            const int fa = c.a0 + warp + p_a * W;
+            const int q = (int)((unsigned)fa / (unsigned)ncw), cell = fa - q * ncw;
+            tile0 = (p.base * nb + q) * R;
+            p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
+            p_left = 1;
+            ++p_a;
+        } else if (!p_b_started) {                                          // phase B starts: cell bs of the CTA's whole units
+            p_b_started = true;
+            const int ul = (int)((unsigned)bs / (unsigned)ncw), cell = bs - ul * ncw;
+            tile0 = (c.unit0 + ul) * R;
+            p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
+            p_left = ncw - cell;
+        } else {                                                            // next whole unit of the run
+            p_src += unit_jump;
+            p_left = ncw;
+            tile0 = (int)((p_src - p.blob) / tile_stride);
+        }
+        p_nv = p.ntiles - tile0; p_nv = p_nv > R ? R : p_nv;
+    };
     auto issue = [&]() {
         mbar_arrive_expect_tx(p_bar, (uint32_t)p_nv * CELL_BYTES);
 #pragma unroll
@@ -770,38 +869,85 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
             if (r < p_nv) bulk_g2s(p_dst + r * CELL_BYTES, p_src + r * tile_stride, CELL_BYTES, p_bar);
         ++p_count;
         p_src += CELL_BYTES;
-        if (--p_left == 0) {                                                // next unit of the share
-            p_src += unit_jump;
-            p_left = ncw;
-            if (R > 1) { p_nv = p.ntiles - (int)((p_src - p.blob) / tile_stride); p_nv = p_nv > R ? R : p_nv; }
-        }
+        if (--p_left == 0) next_run();
         p_dst += STAGE_BYTES; p_bar += 8;
         if (p_dst == ring_end) { p_dst -= (uint32_t)S * STAGE_BYTES; p_bar -= (uint32_t)S * 8; }
     };
-    uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
-    if (leader) {                                                           // start the weight stream first
+    if (leader) {
         for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
         mbar_fence_init();
+        if (total > 0) next_run();
         const int npre = total < S ? total : S;
         for (int i = 0; i < npre; ++i) issue();
-        hdr = __ldg(reinterpret_cast<const uint4*>(p.blob - BLOB_HEADER_BYTES));    // checked before the first output
     }
+    if (threadIdx.x == 0) NVFP4_TRACE(1);
+
+    // ---- CTA-wide tables and barriers ----
+    for (int i = threadIdx.x; i < p.base + 3; i += blockDim.x) cnt[i] = 0;
+    if (threadIdx.x <= W) bstart[threadIdx.x] = Bc - (int)(((unsigned)(W - threadIdx.x) * (unsigned)Bc) / (unsigned)W);
+    for (unsigned b = threadIdx.x; b <= (unsigned)nb; b += blockDim.x) {
+#pragma unroll
+        for (int v = 0; v < 2; ++v) {
+            const unsigned nba = (unsigned)p.nba[v];
+            const unsigned bb = b < nba ? b : nba;                          // CTAs that take no part repeat the end
+            astart[v * (nb + 1) + b] = nba ? (int)(bb * (unsigned)p.a_q[v] + (bb * (unsigned)p.a_r[v]) / nba) : 0;
+        }
+    }
+    for (int i = threadIdx.x; i < p.nxb; i += blockDim.x) mbar_init(smem_u32(xbars + i), blockDim.x);
+    for (int i = threadIdx.x; i < p.nhand; i += blockDim.x) mbar_init(smem_u32(hbars + i), 1);
+    if (threadIdx.x == 0) mbar_fence_init();
+    __syncthreads();
+
+    // a blob that was not repacked for this (N, K, KP, ABI version) must not produce plausible numbers: one thread
+    // per CTA checks the header; the flag is published by its first staging-barrier arrival
+    uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
+    const bool checker = (threadIdx.x == W * 32);
+    if (checker) hdr = __ldg(reinterpret_cast<const uint4*>(p.blob - BLOB_HEADER_BYTES));
     // the weight stream is under way; everything below touches data of the previous kernel
     pdl_wait();
     pdl_launch_dependents();
+    if (threadIdx.x == 0) NVFP4_TRACE(2);
+    if (checker)
+        *blob_flag = (hdr.x == p.hdr_expect.x) && (hdr.y == p.hdr_expect.y) && (hdr.z == p.hdr_expect.z) &&
+                     (hdr.w == p.hdr_expect.w);
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
-    if (fused)      // consumers take their share of the quantization while their first weight cells are in flight
-        stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
     const float gx_raw = (MODE == KMODE_W4A16 || fused || p.gscale_per_row) ? 1.0f : __ldg(p.x_gscale);
+    // activation staging: every thread of the CTA takes its share
+    if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars);
+    else if (fused)          stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
+    else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars);
+    if (threadIdx.x == W * 32) NVFP4_TRACE(9);
 
+    if (!consumer) {                                                        // ---- closer warps ----
+        // units this CTA holds only a part of: the (at most two) leftover units, and with K slices every whole unit
+        const int sw = warp - W, nsw = (int)(blockDim.x >> 5) - W;
+        const int njobs = 2 + (p.ksplit > 1 ? my_base : 0);
+        for (int j = sw; j < njobs; j += nsw) {
+            if (j == 0 && (c.n0 == 0 || (p.ksplit == 1 && c.n0 == ncw))) continue;
+            if (j == 1 && c.na - c.n0 == 0) continue;                       // (a second leftover unit is never whole)
+            mbar_wait(smem_u32(hbars + j), 0u);
+            float g = gw_raw;
+            if (MODE != KMODE_W4A16) {
+                g = g * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw);
+                if (MODE == KMODE_W4A4_I8) g *= 0.25f;                       // ints are 2*e (exact scaling)
+            }
+            if (!*blob_flag) g = __int_as_float(0x7FC00000);
+            if (lane == 0) NVFP4_TRACE(10 + (j & 1) * 2);
+            close_unit<M, R>(p, c, hand + (size_t)j * (R * M * rpt), j < 2, j < 2 ? c.qa0 + j : j - 2, lane, rpt, g);
+            if (lane == 0) NVFP4_TRACE(11 + (j & 1) * 2);
+        }
+        return;
+    }
+
+    // ---- consumer warps ----
     float acc[R][M];
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
         for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
 
-    uint64_t accp[R][M];                       // integer path: packed {even blocks, odd blocks} partial sums
+    uint64_t accp[R][M];                       // W4A4 paths: packed {even blocks, odd blocks} partial sums
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -811,30 +957,47 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     // this lane's activation records: vector (cell*8 + j)*kp + part  ->  stride between j steps = kp records
     const size_t xstep = (size_t)p.kp * XVS;
     const uint8_t* xlane0 = xs + (size_t)part * XVS;
-    int c_ul = f0_ul;
-    const int cell0 = f0 - c_ul * ncw;
-    const uint8_t* xlane = xlane0 + (size_t)cell0 * CELL_VECS * xstep;
-    // loop state kept incremental (no per-iteration index arithmetic): consumer stage pointer and
-    // barrier, cells left in the current segment, staging items this lane's next cell depends on
+    constexpr int ITEMS_PER_CELL_KP = M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2); // staging items per cell and K part
+    const int x_items_cell = p.kp * ITEMS_PER_CELL_KP;
+    // loop state kept incremental: consumer stage pointer and barrier, cells left in the current segment,
+    // staging items this lane's next cell depends on
     const uint8_t* st = ring;
     const uint8_t* const st_end = ring + (size_t)S * STAGE_BYTES;
     uint32_t bar = smem_u32(bars);
     uint32_t phase = 0;
-    int seg_left = (ncw - cell0) < total ? (ncw - cell0) : total;           // cells until the segment ends
-    bool seg_first = true, seg_from0 = (cell0 == 0);
-    constexpr int ITEMS_PER_CELL_KP = M * CELL_VECS * ((MODE == KMODE_W4A16) ? 4 : 2); // staging items per cell and K part
-    const int x_items_cell = p.kp * ITEMS_PER_CELL_KP;
-    int x_need = (cell0 + 1) * x_items_cell;                                // items that must be staged
+    // segments: a leftover cell (phase A) is a segment of its own; in phase B a segment ends with its unit
+    int c_ul = 0, seg_left = 0, seg_cell0 = 0, seg_len = 0, a_k = 0;
+    bool seg_first = true, seg_in_a = false, b_started = false;
+    const uint8_t* xlane = xlane0;
+    int x_need = 0;
     int x_have = 0;                                                         // items known to be staged
     uint32_t xbar = smem_u32(xbars);
-    // a blob that was not repacked for this (N, K, KP, ABI version) must not produce plausible numbers: NaN outputs
-    hdr.x = __shfl_sync(0xFFFFFFFFu, hdr.x, 0); hdr.y = __shfl_sync(0xFFFFFFFFu, hdr.y, 0);
-    hdr.z = __shfl_sync(0xFFFFFFFFu, hdr.z, 0); hdr.w = __shfl_sync(0xFFFFFFFFu, hdr.w, 0);
-    const bool blob_ok = (hdr.x == p.hdr_expect.x) && (hdr.y == p.hdr_expect.y) && (hdr.z == p.hdr_expect.z) &&
-                         (hdr.w == p.hdr_expect.w);
+    auto next_segment = [&](int left) {                                     // left = cells of this warp still to do (> 0)
+        int cell;
+        if (a_k < na_w) {
+            const int fa = c.a0 + warp + a_k * W;
+            cell = fa - (int)((unsigned)fa / (unsigned)ncw) * ncw;
+            seg_in_a = true; seg_len = 1;
+        } else if (!b_started) {
+            b_started = true; seg_in_a = false;
+            c_ul = (int)((unsigned)bs / (unsigned)ncw);
+            cell = bs - c_ul * ncw;
+            seg_len = ncw - cell < left ? ncw - cell : left;
+        } else {
+            ++c_ul; cell = 0;
+            seg_len = ncw < left ? ncw : left;
+        }
+        seg_cell0 = cell; seg_left = seg_len;
+        xlane = xlane0 + (size_t)cell * CELL_VECS * xstep;
+        x_need = (cell + 1) * x_items_cell;
+    };
+    if (total > 0) next_segment(total);
     for (int f = 0; f < total; ++f) {
         while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += stage_items; }
+        if (threadIdx.x == 0 && f == 0) NVFP4_TRACE(3);
         mbar_wait(bar, phase);
+        if (threadIdx.x == 0 && f < 3) NVFP4_TRACE(4 + f);
+        if (lane == 0 && f == 1) NVFP4_TRACE(40 + warp);
 
 #pragma unroll
         for (int hc = 0; hc < CELL_VECS / 4; ++hc) {                       // half cells: 8 scales, 4 vectors
@@ -849,7 +1012,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
                 const float2 f3s = e4m3x2_to_float2((uint16_t)(sc.y >> 16));
                 sw[r][0] = f0s.x; sw[r][1] = f0s.y; sw[r][2] = f1s.x; sw[r][3] = f1s.y;
                 sw[r][4] = f2s.x; sw[r][5] = f2s.y; sw[r][6] = f3s.x; sw[r][7] = f3s.y;
-                if (MODE == KMODE_W4A4_I8) {
+                if (MODE != KMODE_W4A16) {
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
                         swp[r][q] = pack2u(__float_as_uint(sw[r][2 * q]), __float_as_uint(sw[r][2 * q + 1]));
@@ -863,7 +1026,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
                     wv[r] = *reinterpret_cast<const uint4*>(st + r * CELL_BYTES + (hc * 4 + j) * 512 + lane * 16);
                 const uint8_t* xbp = xlane + (size_t)(hc * 4 + j) * xstep;
                 if (MODE == KMODE_W4A4_I8)     block_pair_w4a4<M, R>(lut, wv, xbp, swp, j, accp);
-                else if (MODE == KMODE_W4A4_H) block_pair_w4a4_h<M, R>(wv, xbp, sw, j, acc);
+                else if (MODE == KMODE_W4A4_H) block_pair_w4a4_h<M, R>(wv, xbp, swp, j, accp);
                 else                           block_pair_w4a16<M, R>(wv, xbp, sw, j, acc);
             }
         }
@@ -877,7 +1040,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         if (st == st_end) { st = ring; bar -= (uint32_t)S * 8; phase ^= 1u; }
 
         if (--seg_left == 0) {                                              // segment finished
-            if (MODE == KMODE_W4A4_I8) {
+            if (MODE != KMODE_W4A16) {
 #pragma unroll
                 for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -890,20 +1053,26 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
             float gs = gw_raw;
             if (MODE == KMODE_W4A4_I8) gs = (gs * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw)) * 0.25f;   // ints are 2*e
             if (MODE == KMODE_W4A4_H)  gs = gs * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw);
-            if (!blob_ok) gs = __int_as_float(0x7FC00000);
+            if (!*blob_flag) gs = __int_as_float(0x7FC00000);               // (published before the first staging barrier)
             const int left = total - f - 1;
-            const bool unit_end = (left == 0) ? (x_need - x_items_cell == ncw * x_items_cell) : true;
-            finish_segment<M, R>(p, c, acc, slots, cnt, fstart, c_ul, seg_from0 && unit_end, seg_first,
-                                 warp, lane, part, rsub, rpt, gs);
+            if (seg_in_a) {
+                finish_leftover_cell<M, R>(p, c, acc, aslots, hand, hbars, cnt, warp + a_k * W, lane, part, rsub, rpt, gs);
+                ++a_k;
+            } else {
+                const bool whole = (seg_cell0 == 0) && (seg_len == ncw);
+                finish_segment<M, R>(p, c, acc, slots, hand, hbars, cnt, bstart, c_ul, whole, seg_first,
+                                     warp, lane, part, rsub, rpt, gs);
+                seg_first = false;
+            }
+            if (left > 0) next_segment(left);
 #pragma unroll
             for (int r = 0; r < R; ++r)
 #pragma unroll
                 for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
-            seg_first = false; seg_from0 = true;
-            seg_left = left < ncw ? left : ncw;
-            ++c_ul; xlane = xlane0; x_need = x_items_cell;
         }
     }
+    if (lane == 0 && (warp == 0 || warp == W - 1)) NVFP4_TRACE(warp == 0 ? 7 : 14);
+    if (lane == 0) NVFP4_TRACE(16 + warp);
 }
 
 }  // namespace nvfp4

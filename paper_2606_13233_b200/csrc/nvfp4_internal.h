@@ -16,6 +16,9 @@ struct GemvConfig {
     int rows;     // R: row tiles (32/KP rows each) per warp step (1 or 2): x records are loaded once per R tiles
     int stages;   // depth of each warp's private bulk-copy ring (R cells of 4608 B per stage)
     int ksplit;   // number of K slices (grid.y); each slice's activations are staged by its own CTAs
+    int whole;    // 1: whole units only (CTAs get base or base + 1 units, no leftover stream); 0: data-parallel + stream-K
+    int cps;      // CTAs per SM (1..3): with >= 2 the next kernel's CTAs become resident (and prefetch their first
+                  // weight cells) while this kernel's are still running -- programmatic dependent launch
 };
 
 // launch attribute that lets a kernel start before its stream predecessor has finished (PDL)

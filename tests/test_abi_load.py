@@ -69,20 +69,21 @@ def test_argument_validation_without_gpu(lib):
 
 def test_config_table_is_sane(lib):
     ip = ctypes.POINTER(ctypes.c_int)
-    lib.nvfp4_gemv_get_config.argtypes = [ctypes.c_int] * 4 + [ip] * 4
+    lib.nvfp4_gemv_get_config.argtypes = [ctypes.c_int] * 4 + [ip] * 6
     lib.nvfp4_gemv_workspace_bytes.restype = ctypes.c_size_t
     for N, K in [(2048, 2048), (10240, 5120), (5120, 8192), (51200, 5120), (5120, 25600), (1, 16), (100, 208)]:
         for M in range(1, 9):
             for mode in (0, 1):
-                v = [ctypes.c_int(0) for _ in range(4)]
+                v = [ctypes.c_int(0) for _ in range(6)]
                 assert lib.nvfp4_gemv_get_config(mode, M, N, K, *[ctypes.byref(a) for a in v]) == 0
-                ks, warps, rows, stages = [a.value for a in v]
-                assert 1 <= ks <= (K + 255) // 256 and 1 <= warps <= 20 and rows in (1, 2) and 1 <= stages <= 16
+                ks, warps, rows, stages, cps, bal = [a.value for a in v]
+                assert 1 <= ks <= (K + 255) // 256 and 1 <= warps <= 20 and rows in (1, 2) and 1 <= stages <= 16 and 1 <= cps <= 3 and bal in (1, 2)
             assert lib.nvfp4_gemv_workspace_bytes(M, N, K) > 0
-    assert lib.nvfp4_gemv_set_config(0, 0, 3, 0) == -1
-    assert lib.nvfp4_gemv_set_config(0, 0, 4, 0) == -1
+    assert lib.nvfp4_gemv_set_config(0, 0, 3, 0, 0, 0) == -1
+    assert lib.nvfp4_gemv_set_config(0, 0, 4, 0, 0, 0) == -1 and lib.nvfp4_gemv_set_config(0, 0, 0, 0, 4, 0) == -1
+    assert lib.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 3) == -1
     assert lib.nvfp4_set_layout_kparts(3) == -1 and lib.nvfp4_set_layout_kparts(64) == -1
     assert lib.nvfp4_set_layout_kparts(4) == 0 and lib.nvfp4_get_layout_kparts(5120, 5120) == 4
     assert lib.nvfp4_set_layout_kparts(0) == 0 and lib.nvfp4_get_layout_kparts(5120, 25600) == 4
     assert lib.nvfp4_get_layout_kparts(51200, 5120) == 1
-    assert lib.nvfp4_gemv_set_config(0, 0, 0, 0) == 0
+    assert lib.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0) == 0

@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 @pytest.fixture(scope="module")
 def B():
     from paper_2606_13233_b200 import binding
-    binding.nvfp4_gemv_set_config(0, 0, 0, 0)
+    binding.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0)
     return binding
 
 

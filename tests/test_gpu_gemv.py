@@ -18,7 +18,7 @@ pytestmark = pytest.mark.gpu
 def B():
     from paper_2606_13233_b200 import binding
     yield binding
-    binding.nvfp4_gemv_set_config(0, 0, 0, 0)
+    binding.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0)
 
 
 class Case:
@@ -51,7 +51,13 @@ class Case:
         return y
 
 
-def check_both_dtypes(B, case, mode, bf16_slack=True):
+# The named toy cases whose K is so small that there is no cancellation (|Y| / A > 0.26): for them NO BF16 value can
+# be within 1e-3*A of Y (RN_bf16 of the oracle's own Y already misses it, R9), so the BF16 check adds the
+# BF16 half-ulp there -- and only there; FP32 output is held to the bound as written in every case.
+BF16_SLACK_CASES = {(1, 32, 128), (3, 257, 400), (5, 513, 640), (7, 1000, 384), (8, 31, 48)}
+
+
+def check_both_dtypes(B, case, mode, bf16_slack=False):
     run = case.run_w4a4 if mode == "w4a4" else case.run_w4a16
     Y, A = (case.Y44, case.A44) if mode == "w4a4" else (case.Y416, case.A416)
     y32 = run(B, B.DTYPE_F32)
@@ -124,10 +130,11 @@ SMALL = [(1, 32, 128), (2, 100, 208), (3, 257, 400), (4, 96, 1040), (5, 513, 640
 
 @pytest.mark.parametrize("M,N,K", SMALL)
 def test_small_shapes_both_modes(B, M, N, K):
-    B.nvfp4_gemv_set_config(0, 0, 0, 0)
+    B.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0)
     case = Case(B, M, N, K, seed=1, shape_id=M)
-    check_both_dtypes(B, case, "w4a4")
-    check_both_dtypes(B, case, "w4a16")
+    slack = (M, N, K) in BF16_SLACK_CASES
+    check_both_dtypes(B, case, "w4a4", bf16_slack=slack)
+    check_both_dtypes(B, case, "w4a16", bf16_slack=slack)
     # brute-force dense matmul on the dequantised operands for a few entries (oracle independence)
     vW = orc.dequantize(case.wc, case.ws, case.gw); vX = orc.dequantize(case.xc, case.xs, case.gx)
     n = N // 2
@@ -135,7 +142,8 @@ def test_small_shapes_both_modes(B, M, N, K):
 
 
 @pytest.mark.parametrize("cfg", [(1, 1, 1, 1), (2, 2, 2, 2), (3, 4, 2, 2), (5, 8, 1, 4), (7, 3, 2, 5), (16, 16, 1, 2),
-                                 (4, 1, 2, 8), (64, 2, 2, 3), (1, 16, 2, 2), (2, 20, 1, 3)])
+                                 (4, 1, 2, 8), (64, 2, 2, 3), (1, 16, 2, 2), (2, 20, 1, 3), (1, 6, 1, 2, 2), (2, 4, 2, 2, 2),
+                                 (1, 4, 1, 3, 3), (1, 12, 1, 2, 1, 2), (3, 8, 2, 2, 1, 2), (2, 5, 1, 2, 2, 2), (1, 12, 1, 2, 1, 1)])
 def test_launch_shapes_agree(B, cfg):
     """every split-K / rows / warps / stages combination computes the same thing (ragged shapes:
     N not a multiple of warps*rows*32, K not a multiple of ksplit*128)."""
@@ -146,7 +154,7 @@ def test_launch_shapes_agree(B, cfg):
             check_both_dtypes(B, case, "w4a4")
             check_both_dtypes(B, case, "w4a16")
     finally:
-        B.nvfp4_gemv_set_config(0, 0, 0, 0)
+        B.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0)
 
 
 def test_workspace_reuse_and_determinism(B):
@@ -164,7 +172,7 @@ def test_workspace_reuse_and_determinism(B):
         U.check_gemv(U.host_y_f64(ys[0]), case.Y44, case.A44, "reuse")
         assert int(ws[:256].view(torch.int32).abs().sum()) == 0       # counters back to zero
     finally:
-        B.nvfp4_gemv_set_config(0, 0, 0, 0)
+        B.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0)
 
 
 def test_config0_single_gemv(B):
@@ -186,5 +194,5 @@ def test_config0_single_gemv(B):
 def test_medium_shape_all_m(B, M):
     """several CTA rows, several K ranges, the tuned launch shape, every M of configs[2]."""
     case = Case(B, M, 2048 + 96, 5120, seed=0, shape_id=10 + M)
-    check_both_dtypes(B, case, "w4a4", bf16_slack=False)      # config-like K: tolerance as written
-    check_both_dtypes(B, case, "w4a16", bf16_slack=False)
+    check_both_dtypes(B, case, "w4a4")      # config-like K: tolerance as written
+    check_both_dtypes(B, case, "w4a16")

@@ -108,8 +108,15 @@ def test_bf16_helpers():
     assert np.array_equal(bits, x.astype(ml.bfloat16).view(np.uint16))
     assert np.array_equal(O.bf16_bits_to_f32(bits), x.astype(ml.bfloat16).astype(np.float32))
     y = rng.standard_normal(100000) * 100
-    assert np.array_equal(O.round_to_bf16(y), y.astype(ml.bfloat16).astype(np.float32)) or \
-        np.max(np.abs(O.round_to_bf16(y) - y)) <= np.max(np.abs(y.astype(np.float32).astype(ml.bfloat16).astype(np.float64) - y))
+    # float64 -> BF16 in ONE rounding: nearest BF16 neighbour of every y (brute force over the two candidates
+    # around the truncated bit pattern), ties cannot occur for these random doubles
+    r = O.round_to_bf16(y).astype(np.float64)
+    lo = (y.astype(np.float32).view(np.uint32) & np.uint32(0xFFFF0000)).view(np.float32).astype(np.float64)
+    cand = np.stack([lo, (lo.astype(np.float32).view(np.uint32) + np.uint32(0x10000)).view(np.float32).astype(np.float64),
+                     (lo.astype(np.float32).view(np.uint32) - np.uint32(0x10000)).view(np.float32).astype(np.float64)])
+    best = cand[np.argmin(np.abs(cand - y), axis=0), np.arange(y.size)]
+    assert np.array_equal(r, best)
+    assert np.all(np.abs(r - y) <= np.abs(y) * 2.0 ** -8)        # half an ulp of an 8-bit significand
     # exact ties go to even
     assert O.round_to_bf16(np.array([1.00390625]))[0] == np.float32(1.0)       # 1 + 2^-8 -> 1
     assert O.round_to_bf16(np.array([1.01171875]))[0] == np.float32(1.015625)  # 1 + 3*2^-8 -> 1 + 2^-6

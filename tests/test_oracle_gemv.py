@@ -102,5 +102,11 @@ def test_transposed_operand_would_fail():
 def test_silu_mul():
     gu = np.array([[0.0, 1.0, -2.0, 3.0, 2.0, 0.5, 4.0, -1.0]], dtype=np.float32)
     h = O.silu_mul(gu)
-    want = [0.0 * 2.0, 1 / (1 + np.exp(-1.0)) * 0.5, -2 / (1 + np.exp(2.0)) * 4.0, 3 / (1 + np.exp(-3.0)) * -1.0]
-    np.testing.assert_allclose(h[0], want, rtol=1e-15)
+    # literal constants (40-digit decimal arithmetic, not the oracle's expression):
+    # silu(1) = 0.73105857863000487925..., silu(-2) = -0.23840584404423517..., silu(3) = 2.85772238046729965...
+    want = [0.0, 0.7310585786300048793 * 0.5, -0.2384058440442351119 * 4.0, 2.857722380467299657 * -1.0]
+    np.testing.assert_allclose(h[0], want, rtol=4e-16, atol=0)
+    # silu(-x) = silu(x) - x (identity of the logistic function), and h is odd in `up`
+    x = np.array([[0.375, 2.5, -7.0, 11.0, 1.0, 1.0, 1.0, 1.0]], dtype=np.float32)
+    xm = x.copy(); xm[0, :4] = -xm[0, :4]
+    np.testing.assert_allclose(O.silu_mul(xm)[0], O.silu_mul(x)[0] - x[0, :4].astype(np.float64), rtol=0, atol=4e-15)
