@@ -58,6 +58,8 @@ extern "C" {
 /* nvfp4_quantize_act `gscale_mode` */
 #define NVFP4_GSCALE_DYNAMIC 0 /* g = max|X| / 2688 over the whole [M,K] call argument; WRITTEN to *gscale (R3) */
 #define NVFP4_GSCALE_STATIC  1 /* *gscale is READ (a calibrated value, the paper's deployed flow) */
+#define NVFP4_GSCALE_DYNAMIC_PER_ROW 2 /* per-token variant (R3): gscale[m] = max|X[m,:]| / 2688, M floats WRITTEN;
+                                         feeds nvfp4_gemv_rowscale.  Single-launch sizes only (M*K <= 524288). */
 
 /* ABI version == repacked-blob format version. */
 int nvfp4_version(void);
@@ -188,6 +190,19 @@ int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps
                           int* ctas_per_sm, int* balance);
 int nvfp4_set_layout_kparts(int kparts);
 int nvfp4_get_layout_kparts(int N, int K);
+
+/*
+ * SiLU*mul + activation quantizer in ONE launch (the producer of down_proj's input in
+ * BASELINE.json configs[4]):  h[m,j] = RN_bf16(silu(gu[m,j]) * gu[m,I+j])  (same FP32 expression and BF16 rounding
+ * as nvfp4_silu_mul), then the NVFP4 quantizer of nvfp4_quantize_act on h[M,I].  codes / scales / gscale are
+ * bit-identical to nvfp4_silu_mul followed by nvfp4_quantize_act; the BF16 intermediate is not written unless
+ * h_bf16_opt is given.
+ *   gu_bf16 [device] BF16 [M, 2I], row stride 2I;  I % 16 == 0, M*I <= 524288
+ *   codes [device] out uint8 [M, I/2];  scales [device] out uint8 [M, I/16];  gscale as for nvfp4_quantize_act
+ *   h_bf16_opt [device] optional (may be NULL): BF16 [M, I] copy of the intermediate
+ */
+int nvfp4_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, uint8_t* scales, float* gscale,
+                            int gscale_mode, void* h_bf16_opt, void* stream);
 
 /*
  * Glue of the decode chain (step a8, BASELINE.json configs[4]; not part of the paper's kernel):

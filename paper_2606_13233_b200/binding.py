@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_PKG, "libnvfp4_b200.so")
 
 MODE_W4A4, MODE_W4A16 = 0, 1
 DTYPE_F32, DTYPE_BF16 = 0, 1
-GSCALE_DYNAMIC, GSCALE_STATIC = 0, 1
+GSCALE_DYNAMIC, GSCALE_STATIC, GSCALE_DYNAMIC_PER_ROW = 0, 1, 2
 ERR_NAMES = {0: "NVFP4_OK", -1: "NVFP4_ERR_INVALID_ARG", -2: "NVFP4_ERR_UNSUPPORTED_SHAPE",
              -3: "NVFP4_ERR_ALIGNMENT", -4: "NVFP4_ERR_CUDA"}
 
@@ -25,7 +25,7 @@ ERR_NAMES = {0: "NVFP4_OK", -1: "NVFP4_ERR_INVALID_ARG", -2: "NVFP4_ERR_UNSUPPOR
 SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp4_repacked_bytes",
            "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
            "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant",
-           "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts")
+           "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts", "nvfp4_silu_mul_quantize")
 
 
 class Nvfp4Error(RuntimeError):
@@ -69,6 +69,8 @@ def _load():
     lib.nvfp4_gemv_set_config.argtypes = [c_int, c_int, c_int, c_int, c_int, c_int]
     lib.nvfp4_gemv_get_config.restype = c_int
     lib.nvfp4_gemv_get_config.argtypes = [c_int, c_int, c_int, c_int] + [ctypes.POINTER(c_int)] * 6
+    lib.nvfp4_silu_mul_quantize.restype = c_int
+    lib.nvfp4_silu_mul_quantize.argtypes = [vp, c_int, c_int, vp, vp, vp, c_int, vp, vp]
     lib.nvfp4_silu_mul.restype = c_int
     lib.nvfp4_silu_mul.argtypes = [vp, c_int, c_int, vp, vp]
     return lib
@@ -103,7 +105,7 @@ def nvfp4_quantize_act(x_bf16, codes=None, scales=None, gscale=None, gscale_mode
     if scales is None:
         scales = torch.empty((M, K // 16), dtype=torch.uint8, device=dev)
     if gscale is None:
-        gscale = torch.zeros(1, dtype=torch.float32, device=dev)
+        gscale = torch.zeros(M if gscale_mode == GSCALE_DYNAMIC_PER_ROW else 1, dtype=torch.float32, device=dev)
     _check(lib.nvfp4_quantize_act(_ptr(x_bf16), M, K, x_bf16.stride(0), _ptr(codes), _ptr(scales), _ptr(gscale),
                                   gscale_mode, None, 0, _stream()))
     return codes, scales, gscale
@@ -193,6 +195,22 @@ def nvfp4_set_layout_kparts(kparts=0):
 
 def nvfp4_get_layout_kparts(N, K) -> int:
     return lib.nvfp4_get_layout_kparts(N, K)
+
+
+def nvfp4_silu_mul_quantize(gu_bf16, codes=None, scales=None, gscale=None, gscale_mode=GSCALE_DYNAMIC, h=None):
+    """gu_bf16 [M,2I] -> NVFP4 of h = RN_bf16(silu(gate) * up) in one launch: (codes [M,I/2], scales [M,I/16], g)."""
+    M, I2 = gu_bf16.shape
+    I = I2 // 2
+    dev = gu_bf16.device
+    if codes is None:
+        codes = torch.empty((M, I // 2), dtype=torch.uint8, device=dev)
+    if scales is None:
+        scales = torch.empty((M, I // 16), dtype=torch.uint8, device=dev)
+    if gscale is None:
+        gscale = torch.zeros(M if gscale_mode == GSCALE_DYNAMIC_PER_ROW else 1, dtype=torch.float32, device=dev)
+    _check(lib.nvfp4_silu_mul_quantize(_ptr(gu_bf16), M, I, _ptr(codes), _ptr(scales), _ptr(gscale), gscale_mode, _ptr(h),
+                                       _stream()))
+    return codes, scales, gscale
 
 
 def nvfp4_silu_mul(gu_bf16, h=None):

@@ -19,8 +19,11 @@ QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
 
 
 class DecodeChain:
-    def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False):
+    def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False,
+                 fused_producer: bool = True):
         self.fused = fused                            # one nvfp4_gemv_fused_quant launch per projection
+        self.fused_producer = fused_producer          # down's input: nvfp4_silu_mul_quantize (one launch) instead of
+                                                      # nvfp4_silu_mul + nvfp4_quantize_act
         d = dict(QWEN3_32B_DIMS if dims is None else dims)
         self.M, self.layers, self.d = M, layers, d
         H, QKV, OIN, I = d["hidden"], d["qkv"], d["o_in"], d["inter"]
@@ -48,10 +51,18 @@ class DecodeChain:
         self.xs = torch.empty((M, kmax // 16), dtype=u8, device=device)
         self.gx = torch.zeros(1, dtype=torch.float32, device=device)
         self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
-        self.launches_per_step = layers * (5 if fused else 9)
+        self.launches_per_step = layers * ((5 if fused else 8) if fused_producer else (5 if fused else 9))
 
     def set_input(self, h_bf16):
         self.h.copy_(h_bf16)
+
+    def _down_from_gate_up(self, l, y, keep_h=False):
+        """down projection fed by the fused producer: SiLU*mul + quantize in one launch, then the W4A4 GEMV."""
+        blob, gw, N, K = self.w[l][3]
+        xc = self.xc.view(-1)[: self.M * (K // 2)].view(self.M, K // 2)
+        xs = self.xs.view(-1)[: self.M * (K // 16)].view(self.M, K // 16)
+        B.nvfp4_silu_mul_quantize(self.y_gu, xc, xs, self.gx, h=self.act if keep_h else None)
+        B.nvfp4_gemv(B.MODE_W4A4, blob, gw, N, K, xc, xs, self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[3])
 
     def _proj(self, l, i, x, y):
         blob, gw, N, K = self.w[l][i]
@@ -70,9 +81,12 @@ class DecodeChain:
             stages = (("qkv", self.h, self.y_qkv), ("o", self.y_qkv[:, : d["o_in"]], self.y_o),
                       ("gate_up", self.y_o, self.y_gu), ("down", self.act, self.h))
             for i, (name, x, y) in enumerate(stages):
-                if name == "down":
-                    B.nvfp4_silu_mul(self.y_gu, self.act)
-                self._proj(l, i, x, y)
+                if name == "down" and self.fused_producer:
+                    self._down_from_gate_up(l, y, keep_h=taps is not None)
+                else:
+                    if name == "down":
+                        B.nvfp4_silu_mul(self.y_gu, self.act)
+                    self._proj(l, i, x, y)
                 if taps is not None:
                     taps.append((l, name, x.clone(), y.clone()))
 

@@ -61,8 +61,10 @@ int nvfp4_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* c
     (void)workspace; (void)ws_bytes;
     g_last_err[0] = 0;
     if (!x_bf16 || !codes || !scales || !gscale) return NVFP4_ERR_INVALID_ARG;
-    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC &&
+        gscale_mode != NVFP4_GSCALE_DYNAMIC_PER_ROW) return NVFP4_ERR_INVALID_ARG;
     if (!shape_ok(M, 1, K) || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (gscale_mode == NVFP4_GSCALE_DYNAMIC_PER_ROW && (int64_t)M * K > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     if (!aligned16(x_bf16) || !aligned16(codes) || !aligned16(scales) || (reinterpret_cast<uintptr_t>(gscale) & 3u))
         return NVFP4_ERR_ALIGNMENT;
     cudaError_t e = launch_quantize_act(x_bf16, M, K, ldx, codes, scales, gscale, gscale_mode,
@@ -200,6 +202,20 @@ int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps
 int nvfp4_debug_set_trace(void* device_buffer) {
     g_trace = static_cast<unsigned long long*>(device_buffer);
     return NVFP4_OK;
+}
+
+int nvfp4_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, uint8_t* scales, float* gscale,
+                            int gscale_mode, void* h_bf16_opt, void* stream) {
+    g_last_err[0] = 0;
+    if (!gu_bf16 || !codes || !scales || !gscale) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC &&
+        gscale_mode != NVFP4_GSCALE_DYNAMIC_PER_ROW) return NVFP4_ERR_INVALID_ARG;
+    if (!shape_ok(M, 1, I) || (int64_t)M * I > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(gu_bf16) || !aligned16(codes) || !aligned16(scales) || (h_bf16_opt && !aligned16(h_bf16_opt)) ||
+        (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_silu_mul_quantize(gu_bf16, M, I, codes, scales, gscale, gscale_mode, h_bf16_opt,
+                                             static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
 int nvfp4_silu_mul(const void* gu_bf16, int M, int I, void* h_bf16, void* stream) {

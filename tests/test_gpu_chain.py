@@ -11,12 +11,13 @@ import _gpu_util as U
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("M,fused", [(1, False), (4, False), (1, True), (2, True)])
-def test_chain_small_dims_every_stage(M, fused):
+@pytest.mark.parametrize("M,fused,producer", [(1, False, True), (4, False, True), (1, True, True), (2, True, True),
+                                              (3, False, False), (1, True, False)])
+def test_chain_small_dims_every_stage(M, fused, producer):
     from paper_2606_13233_b200 import binding as B
     from paper_2606_13233_b200.chain import DecodeChain
     dims = dict(hidden=256, qkv=512, o_in=384, inter=512)
-    ch = DecodeChain(layers=3, M=M, dims=dims, seed=5, fused=fused)
+    ch = DecodeChain(layers=3, M=M, dims=dims, seed=5, fused=fused, fused_producer=producer)
     ch.calibrate(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77)))
     taps = []
     ch.step(taps)
@@ -30,7 +31,7 @@ def test_chain_small_dims_every_stage(M, fused):
         assert np.all(np.isfinite(xf))
         oxc, oxs, ogx = orc.quantize(xf)
         Y, A = orc.gemv_w4a4(U.host_u8(wc), U.host_u8(ws), np.float32(gw.item()), oxc, oxs, ogx)
-        U.check_gemv(U.host_y_f64(y), Y, A, f"layer {l} {name}", bf16_slack=True)
+        U.check_gemv(U.host_y_f64(y), Y, A, f"layer {l} {name}", bf16_slack=True)      # toy K (256..512): no cancellation, R9
         if name == "gate_up":       # the glue that feeds `down`
             assert np.all(np.isfinite(U.host_y_f64(y)))
             want = orc.silu_mul(orc.bf16_bits_to_f32(U.host_bf16_bits(y)))
@@ -46,4 +47,48 @@ def test_chain_small_dims_every_stage(M, fused):
     with torch.cuda.graph(g):
         ch.step()
     ch.set_input(h0); g.replay(); torch.cuda.synchronize()
+    assert torch.equal(ch.h, ref)
+
+
+@pytest.mark.parametrize("M", [1, 4])
+def test_chain_full_size_first_and_last_layer(M):
+    """BASELINE.json configs[4] at full size: 64 layers x {QKV, O, gate_up, down} of the Qwen3-32B shapes, distinct
+    weights per layer (17.5 GB).  Layer 0's four projections and the last layer's are checked against the oracle
+    run on those projections' own downloaded inputs and unpacked weight bytes (sampled rows), tolerance as
+    written (no BF16 slack)."""
+    from paper_2606_13233_b200 import binding as B
+    from paper_2606_13233_b200.chain import DecodeChain
+    L = 64
+    ch = DecodeChain(layers=L, M=M, seed=9)
+    ch.calibrate(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 5120, 0, 78)))
+    taps = []
+    ch.step(taps)
+    torch.cuda.synchronize()
+    assert len(taps) == 4 * L
+    rng = np.random.default_rng(M)
+    for l, name, x, y in taps:
+        if l not in (0, L - 1):
+            continue
+        i = [s[0] for s in ch.shapes].index(name)
+        blob, gw, N, K = ch.w[l][i]
+        wc, ws = B.nvfp4_unpack_weight(blob, N, K)
+        rows = np.unique(np.concatenate([np.array([0, 31, 32, N - 1]), rng.integers(0, N, size=60)]))
+        d_rows = torch.from_numpy(rows).cuda()
+        hw, hs = U.host_u8(wc[d_rows]), U.host_u8(ws[d_rows])
+        del wc, ws
+        xf = orc.bf16_bits_to_f32(U.host_bf16_bits(x.contiguous()))
+        assert np.all(np.isfinite(xf)) and np.any(xf != 0)
+        oxc, oxs, ogx = orc.quantize(xf)
+        Y, A = orc.gemv_w4a4(hw, hs, np.float32(gw.item()), oxc, oxs, ogx)
+        U.check_gemv(U.host_y_f64(y)[:, rows], Y, A, f"full-size chain layer {l} {name} M={M}")
+    assert torch.isfinite(ch.h.float()).all()
+    # graph replay of the whole 64-layer chain reproduces the eager bits
+    h0 = U.dev_bf16_from_bits(inputs.make_activation_bits(M, 5120, 0, 78))
+    ch.set_input(h0); ch.step(); torch.cuda.synchronize()
+    ref = ch.h.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        ch.set_input(h0)
+        ch.step()
+    g.replay(); torch.cuda.synchronize()
     assert torch.equal(ch.h, ref)
