@@ -17,6 +17,9 @@ projection, north_star) / time, i.e. achieved GB/s of the whole step including t
 `e2e` runs the same step through the public Python API from pinned HOST buffers (H2D of the BF16
 activations and D2H of the BF16 outputs inside the timed region).
 `--impl reference` times the CPU oracle (test infrastructure) on a bounded sample.
+The same run also fills `per_m` (the whole BASELINE.json metric: the step and every projection at M = 1, 2, 4, 8, with
+W4A16 and cuBLAS BF16 beside the W4A4 numbers), `chain` (configs[4] at M = 1), and `roofline_alu_m8` (the integer
+path's FMA-heavy-pipe roofline at M = 8).  `--headline-only` skips those legs.
 `--sweep` additionally prints per-shape / per-M tables (cold and warm L2, W4A16, cuBLAS BF16) as
 extra lines BEFORE the final JSON line, for profiles/.
 """
@@ -293,6 +296,105 @@ def job_value(bytes_per_rank_step, world, ms_step):
 
 
 # ---- our arm -----------------------------------------------------------------------------------
+MS = (1, 2, 4, 8)                      # BASELINE.json metric: "at M = 1, 2, 4, 8"
+MIN_REPLAYS = 200                      # timed graph replays, whatever --steps says
+HEAVY_LANES_PER_CLK_SM = 64.0          # IDP.4A / FFMA2 / HFMA2 issue rate (profiles/r02_microbench.md)
+NUM_SMS = 148
+
+
+class ShapeBank:
+    """>= 4 x L2 of DISTINCT repacked copies of one projection's weight (cold-L2 per-shape timing), shared by every
+    M and mode; plus BF16 copies of the same shape for the cuBLAS comparator."""
+
+    def __init__(self, sid, name, N, K):
+        import torch
+        from paper_2606_13233_b200 import binding as B
+        self.torch, self.B, self.sid, self.name, self.N, self.K = torch, B, sid, name, N, K
+        wbytes = N * K * 9 // 16
+        self.copies = max(2, -(-4 * L2_BYTES // wbytes))
+        self.blobs = []
+        for c in range(self.copies):
+            codes, scales, g = inputs.make_nvfp4_weight_device(N, K, seed=c, shape_id=sid)
+            self.blobs.append(B.nvfp4_repack_weight(codes, scales))
+            del codes, scales
+        self.gw = torch.tensor([g], dtype=torch.float32, device="cuda")
+
+    def time_mode(self, M, mode, reps_total=MIN_REPLAYS):
+        """cold-L2 us per call of nvfp4_gemv(mode) at M rows: one graph walks all copies."""
+        torch, B, N, K = self.torch, self.B, self.N, self.K
+        xbits = inputs.make_activation_bits(M, K, seed=0, shape_id=self.sid)
+        x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
+        y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+        ws = B.new_workspace(M, N, K)
+        if mode == "w4a4":
+            xc, xs, gx = B.nvfp4_quantize_act(x)
+            call = lambda b: B.nvfp4_gemv(B.MODE_W4A4, b, self.gw, N, K, xc, xs, gx, y=y, y_dtype=B.DTYPE_BF16, workspace=ws)
+        else:
+            call = lambda b: B.nvfp4_gemv(B.MODE_W4A16, b, self.gw, N, K, x, y=y, y_dtype=B.DTYPE_BF16, workspace=ws)
+        for b in self.blobs[:2]:
+            call(b)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for b in self.blobs:
+                call(b)
+        us = time_graph(torch, g, max(3, reps_total // self.copies), 3) / self.copies * 1e3
+        del g
+        return us
+
+    def time_cublas(self, Ms):
+        """torch.matmul (cuBLAS) BF16 on BF16 weights of the same shape, same cold rotation: {M: us}."""
+        torch, N, K = self.torch, self.N, self.K
+        ncopy = max(2, -(-4 * L2_BYTES // (2 * N * K)))
+        Ws = [torch.randn(N, K, device="cuda", dtype=torch.bfloat16) * 0.02 for _ in range(ncopy)]
+        out = {}
+        for M in Ms:
+            x = torch.randn(M, K, device="cuda", dtype=torch.bfloat16)
+            y = torch.empty(M, N, device="cuda", dtype=torch.bfloat16)
+            for w in Ws:
+                torch.matmul(x, w.t(), out=y)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                for w in Ws:
+                    torch.matmul(x, w.t(), out=y)
+            out[M] = time_graph(torch, g, max(3, 60 // ncopy), 3) / ncopy * 1e3
+            del g
+        del Ws
+        torch.cuda.empty_cache()
+        return out
+
+
+def chain_ms_per_token(M, layers, peak):
+    """BASELINE.json configs[4]: `layers` x {QKV, O, gate_up, down} + quantizers + SiLU*mul, distinct weights per layer,
+    one CUDA graph; the best of the chain's launch variants is reported with its name."""
+    import torch
+    from paper_2606_13233_b200.chain import DecodeChain
+    h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
+    res = {}
+    for label, fused in (("two_calls", False), ("fused_quant", True)):
+        if fused and M > 1:
+            continue
+        ch = DecodeChain(layers=layers, M=M, fused=fused)
+        ch.calibrate(h0)
+        ch.step()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            ch.set_input(h0)               # every replay is the same token (a 10-80 KB device copy)
+            ch.step()
+        ms = time_graph(torch, g, 20, 3)
+        res[label] = {"ms_per_token": round(ms, 4), "launches": ch.launches_per_step,
+                      "frac_of_copy_peak": round(ch.weight_bytes() / ms / 1e6 / peak, 3),
+                      "finite": bool(torch.isfinite(ch.h.float()).all())}
+        wb = ch.weight_bytes()
+        del ch, g
+        torch.cuda.empty_cache()
+    best = min(res, key=lambda k: res[k]["ms_per_token"])
+    return {"M": M, "layers": layers, "weight_gb": round(wb / 1e9, 2), "best": best, **res[best], "variants": res,
+            "floor_ms_at_peak": round(wb / peak / 1e6, 3)}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -304,39 +406,41 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peak, peak_src = measured_peak()
     M = args.m
-    wl = Workload(M, copies=2)
-    # graphs: the whole step (2 copies per replay), the GEMVs alone, the quantizers alone
-    g_step, n_step = wl.capture(2)
-    g_gemv, n_gemv = wl.capture(2, quant=False)
-    g_q, n_q = wl.capture(2, gemv=False)
-    g_fused, n_fused = wl.capture(2, fused=True)
-    reps = max(1, (args.steps + 1) // 2)            # one replay = 2 steps
-    wrep = max(2, (args.warmup + 1) // 2)
+    steps = max(args.steps, 2 * MIN_REPLAYS)         # one replay = 2 steps; never fewer than MIN_REPLAYS replays
+    reps = (steps + 1) // 2
+    wrep = max(3, (args.warmup + 1) // 2)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
+    def time_step_graphs(wl):
+        """(ms/step whole step, ms/step GEMVs alone, ms/step quantizers alone, ms/step fused, launches per replay)"""
+        g_step, n_step = wl.capture(2)
+        g_gemv, _ = wl.capture(2, quant=False)
+        g_q, _ = wl.capture(2, gemv=False)
+        g_fused, _ = wl.capture(2, fused=True)
+        t = [time_graph(torch, g, reps, wrep) / 2 for g in (g_step, g_gemv, g_q, g_fused)]
+        return t[0], t[1], t[2], t[3], n_step
+
+    # ---- headline: the configs[1] step at M rows (default 1) -------------------------------------------------
+    wl = Workload(M, copies=2)
     barrier()
     with ClockSampler(local) as clk:
-        ms_step = time_graph(torch, g_step, reps, wrep) / 2
-        # keep the sampler running over the kernel-only graphs too (same clocks regime)
-        ms_gemv = time_graph(torch, g_gemv, reps, wrep) / 2
-        ms_q = time_graph(torch, g_q, reps, wrep) / 2
-        ms_fused = time_graph(torch, g_fused, reps, wrep) / 2
+        ms_step, ms_gemv, ms_q, ms_fused, n_step = time_step_graphs(wl)
     barrier()
     ms_step = max_over_ranks(ms_step, world, "cuda")
 
-    # end to end through the public API from pinned HOST buffers: per projection H2D of the BF16 activations,
-    # quantize_act, gemv, D2H of the BF16 output -- all inside the timed region.  Measured twice: as plain
-    # stream launches from Python (launch-latency bound) and as a CUDA graph of the same calls + copies
-    # (how a serving loop would replay it); the graph number is the headline `e2e.value`.
+    # end to end through the public API from pinned HOST buffers: H2D of the BF16 activations, quantize_act, gemv,
+    # D2H of the BF16 outputs -- all inside the timed region.  Measured twice: as plain stream launches from Python
+    # (launch-latency bound) and as a CUDA graph of the same calls + copies (how a serving loop would replay it);
+    # the graph number is the headline `e2e.value`.
     for c in range(max(3, args.warmup)):
         wl.step_e2e(c & 1)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    n_eager = min(args.steps, 400)
+    n_eager = min(steps, 400)
     e0.record()
     for i in range(n_eager):
         wl.step_e2e(i & 1)
@@ -350,6 +454,7 @@ def run_ours(args):
     barrier()
     ms_e2e = max_over_ranks(time_graph(torch, g_e2e, reps, wrep) / 2, world, "cuda")
     barrier()
+    del g_e2e
 
     b_step = wl.bytes_step(with_quant=True)
     b_gemv = wl.bytes_step(with_quant=False)
@@ -357,25 +462,59 @@ def run_ours(args):
     ach = b_gemv / (ms_gemv * 1e-3) / 1e9
     h2d = sum(M * p["K"] * 2 for p in wl.proj)
     d2h = sum(M * p["N"] * 2 for p in wl.proj)
+    step_by_m = {M: (ms_step, ms_gemv, ms_q, ms_fused)}
+    del wl
+    torch.cuda.empty_cache()
 
-    per_shape = {}
-    if rank == 0:
-        for p in wl.proj:                               # per-projection cold-L2 numbers (own graphs)
-            g1, _ = wl.capture(2, quant=False, only=p["name"])
-            # a single shape re-read every other launch would be L2-warm for the small ones:
-            # interleave with the full GEMV graph to evict, and subtract it
-            n = 20
-            for _ in range(3):
-                g_gemv.replay(); g1.replay()
-            torch.cuda.synchronize()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            for _ in range(n):
-                g_gemv.replay(); g1.replay()
-            b.record(); torch.cuda.synchronize()
-            us = (a.elapsed_time(b) / n - 2 * ms_gemv) / 2 * 1e3
-            nb = algorithmic_bytes(M, p["N"], p["K"])
-            per_shape[p["name"]] = {"us": round(us, 2), "gbs": round(nb / us / 1e3, 1), "frac": round(nb / us / 1e3 / peak, 3)}
+    per_m, chain, roofline_alu = {}, None, None
+    if rank == 0 and not args.headline_only:
+        # ---- the whole metric: the step at M = 1, 2, 4, 8; per shape W4A4 / W4A16 / cuBLAS BF16, cold L2 --------
+        for m in MS:
+            if m not in step_by_m:
+                w2 = Workload(m, copies=2)
+                step_by_m[m] = time_step_graphs(w2)[:4]
+                del w2
+                torch.cuda.empty_cache()
+        shape_rows = {m: {} for m in MS}
+        for sid, (name, N, K) in enumerate(SHAPES, start=1):
+            bank = ShapeBank(sid, name, N, K)
+            cub = bank.time_cublas(MS)
+            for m in MS:
+                us44 = bank.time_mode(m, "w4a4")
+                us416 = bank.time_mode(m, "w4a16")
+                nb44 = algorithmic_bytes(m, N, K)
+                nb416 = N * K * 9 // 16 + m * K * 2 + m * N * 2
+                shape_rows[m][name] = {
+                    "us": round(us44, 2), "gbs": round(nb44 / us44 / 1e3, 1), "frac": round(nb44 / us44 / 1e3 / peak, 3),
+                    "w4a16_us": round(us416, 2), "w4a16_frac": round(nb416 / us416 / 1e3 / peak, 3),
+                    "cublas_bf16_us": round(cub[m], 2), "copies": bank.copies}
+            del bank
+            torch.cuda.empty_cache()
+        for m in MS:
+            t_step, t_gemv, t_q, t_fused = step_by_m[m]
+            bs = sum(algorithmic_bytes(m, N, K, True) for _, N, K in SHAPES)
+            bg = sum(algorithmic_bytes(m, N, K, False) for _, N, K in SHAPES)
+            per_m[str(m)] = {"ms_per_step": round(t_step, 5), "value": round(bs / (t_step * 1e-3) / 1e9, 1), "unit": UNIT,
+                             "gemv_only_ms": round(t_gemv, 5), "gemv_only_frac": round(bg / (t_gemv * 1e-3) / 1e9 / peak, 3),
+                             "quantize_only_ms": round(t_q, 5), "fused_step_ms": round(t_fused, 5),
+                             "per_shape_gemv": shape_rows[m]}
+        # ---- ALU roofline of the integer path at M = 8 (derivation in DESIGN.md section 7) ----------
+        clk_mhz = clk.summary()["sm_mhz"] or 1965.0
+        weights = sum(N * K for _, N, K in SHAPES)
+        heavy_per_weight = (8 * 8 + 3 * 8) / 32.0                       # 8 dp4a + 3 packed FP32 per (m, 32 weights)
+        ach_alu = heavy_per_weight * weights / (step_by_m[8][1] * 1e-3) / 1e12
+        peak_alu = HEAVY_LANES_PER_CLK_SM * NUM_SMS * clk_mhz * 1e6 / 1e12
+        roofline_alu = {"bound": "alu", "kernel": "gemv_kernel<W4A4 integer path, M=8> (4 launches per step, timed alone)",
+                        "achieved": round(ach_alu, 3), "peak": round(peak_alu, 3), "unit": "T lane-instr/s (FMA-heavy pipe)",
+                        "frac": round(ach_alu / peak_alu, 3), "traffic": None,
+                        "how": "achieved = (8M dp4a + 3M packed FP32)/32 heavy-pipe lane-instructions per weight x weights/s at "
+                               "M = 8; peak = 64 lanes/clk/SM (measured, profiles/r02_microbench.md) x 148 SMs x sampled SM clock",
+                        "hbm_frac_same_kernels": per_m["8"]["gemv_only_frac"]}
+        if not args.no_chain:
+            try:
+                chain = chain_ms_per_token(1, args.layers, peak)
+            except Exception as e:                                        # e.g. not enough free memory on a shared GPU
+                chain = {"unavailable": str(e)[:200]}
 
     cpu = None
     if rank == 0 and not args.no_cpu:
@@ -385,37 +524,45 @@ def run_ours(args):
 
     if rank == 0:
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": ("f16 (HFMA2, exact in-block) + f32 across blocks" if M == 1 else
                       "int8 (dp4a, exact in-block) + f32 across blocks"), "data": "synthetic",
             "config": {"workload": WORKLOAD, "M": M, "l2": "cold: inputs larger than L2 (274 MB weights per step, "
-                       "2 distinct weight sets alternate; L2 = 126 MB)", "timing": "CUDA graph replay, CUDA events",
+                       "2 distinct weight sets alternate; L2 = 126 MB); per-shape numbers walk >= 4 x L2 of distinct copies",
+                       "timing": f"CUDA graph replay, CUDA events, {reps} timed replays of 2 steps (>= {MIN_REPLAYS} whatever --steps)",
                        "multi_gpu": "replicas only"},
             "us_per_projection": {"step_mean": round(ms_step * 1e3 / 4, 2), "gemv_mean": round(ms_gemv * 1e3 / 4, 2),
-                                  "quantize_mean": round(ms_q * 1e3 / 4, 2), "per_shape_gemv": per_shape},
+                                  "quantize_mean": round(ms_q * 1e3 / 4, 2),
+                                  "per_shape_gemv": per_m.get(str(M), {}).get("per_shape_gemv")},
             "fused_step": {"what": "same step with nvfp4_gemv_fused_quant (quantizer inside the GEMV: 4 launches)",
                            "ms_per_step": ms_fused, "value": job_value(b_step, world, ms_fused), "unit": UNIT},
+            "per_m": per_m,
+            "chain": chain,
             "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone)",
                          "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": TRAFFIC_BYTES_PER_STEP.get(M)},
+                         "traffic": TRAFFIC_BYTES_PER_STEP.get(M),
+                         "traffic_source": TRAFFIC_SOURCE if M in TRAFFIC_BYTES_PER_STEP else None},
+            "roofline_alu_m8": roofline_alu,
             "e2e": {"value": job_value(b_step, world, ms_e2e), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "how": "CUDA graph of copies + calls",
                     "eager_value": job_value(b_step, world, ms_e2e_eager), "eager_ms_per_step": ms_e2e_eager},
             "cpu_baseline": cpu,
-            "gpu_launches": n_step // 2 * args.steps if args.steps % 2 == 0 else n_step * reps,
+            "gpu_launches": n_step * reps,
             "clocks": clk.summary(),
         }
         if args.sweep:
-            sweep(wl, peak)
+            sweep(None, peak)
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
 
 
-# per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from
-# the committed `ncu --set full` capture (profiles/); None until a capture exists for that M.
-TRAFFIC_BYTES_PER_STEP = {1: 279.68e6}    # profiles/r01_ncu_full_m1.md (algorithmic: 274.4 MB)
+# per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from the committed
+# `ncu --set full` capture of the same kernels; a constant taken from that file, NOT produced by this run.
+TRAFFIC_BYTES_PER_STEP = {1: 279.68e6}
+TRAFFIC_SOURCE = ("constant from profiles/r02_ncu_full_m1.md (ncu --set full capture of the 4 GEMV launches of this step; "
+                  "algorithmic: 274.4 MB); not measured by this run")
 
 
 def sweep(wl0, peak):
@@ -493,8 +640,9 @@ def run_chain(args):
     import torch
     from paper_2606_13233_b200.chain import DecodeChain
     peak, _ = measured_peak()
-    for M, fused in ((1, False), (2, False), (4, False), (8, False), (1, True), (2, True)):
-        ch = DecodeChain(layers=args.layers, M=M, fused=fused)
+    for M, fused, producer in ((1, False, True), (2, False, True), (4, False, True), (8, False, True), (1, True, True),
+                               (1, False, False), (1, True, False)):
+        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer)
         h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
         ch.calibrate(h0)
         ch.step()
@@ -506,7 +654,7 @@ def run_chain(args):
         ms = time_graph(torch, g, 20, 3)
         finite = bool(torch.isfinite(ch.h.float()).all())
         wb = ch.weight_bytes()
-        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "fused_quant": fused, "ms_per_token": round(ms, 4),
+        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "fused_quant": fused, "fused_producer": producer, "ms_per_token": round(ms, 4),
                           "us_per_layer": round(ms * 1e3 / args.layers, 2), "weight_gb": round(wb / 1e9, 2),
                           "gbs": round(wb / ms / 1e6, 1), "frac_of_copy_peak": round(wb / ms / 1e6 / peak, 3),
                           "launches": ch.launches_per_step, "finite": finite}), flush=True)
@@ -517,12 +665,14 @@ def run_chain(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=4000)
+    ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
     ap.add_argument("--m", type=int, default=1, help="activation rows M (1..8)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sweep", action="store_true", help="also print per-shape / per-M / cuBLAS tables")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-chain", action="store_true", help="skip the configs[4] decode-chain leg (17.5 GB of weights)")
+    ap.add_argument("--headline-only", action="store_true", help="only the configs[1] step at --m rows (no per_m table)")
     ap.add_argument("--profile-shape", default=None, help="qkv|o|gate_up|down|all: plain stream launches of "
                     "quantize_act + gemv on that shape only (for ncu); prints a short JSON line")
     ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16"])
@@ -534,7 +684,7 @@ def main():
     if args.chain:
         return run_chain(args)
     if args.impl == "reference":
-        if args.steps == 4000 and args.warmup == 100:
+        if args.steps == 2000 and args.warmup == 100:
             args.steps, args.warmup = 3, 1
         run_reference(args)
     else:

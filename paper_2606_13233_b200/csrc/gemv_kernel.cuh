@@ -515,7 +515,7 @@ __host__ __device__ inline SmemMap gemv_smem_map(int kmode, int M, int R, int W,
     o = (o + 7u) & ~7u;
     m.bars = o;   o += (uint32_t)W * S * 8;                                // ring mbarriers
     m.xbars = o;  o += (uint32_t)nxb * 8;                                  // staging-batch mbarriers
-    m.hbars = o;  o += (uint32_t)nhand * 8;                                // hand-off mbarriers
+    m.hbars = o;  o += (uint32_t)(nhand + 1) * 8;                          // hand-off mbarriers + the header-check barrier
     m.cnt = o;    o += (uint32_t)(base + 3) * 4;                           // arrival counters: [0,1] leftover units, [2..] whole units
     m.bstart = o; o += (uint32_t)(W + 1) * 4;                              // phase B: warp share starts
     m.astart = o; o += (uint32_t)2 * (nb + 1) * 4;                         // phase A: CTA share starts, both slice variants
@@ -774,6 +774,12 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const int rpt = 32 >> p.kp_shift;
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
     if (threadIdx.x == 0) NVFP4_TRACE(0);
+    // a blob that was not repacked for this (N, K, KP, ABI version) must not produce plausible numbers: one thread
+    // per CTA (the first stager thread) loads the header right away (a cold DRAM access, kept OFF the staging path)
+    // and publishes the verdict through an mbarrier that is checked before the first output is written
+    uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
+    const bool checker = (threadIdx.x == p.warps * 32);
+    if (checker) hdr = __ldg(reinterpret_cast<const uint4*>(p.blob - BLOB_HEADER_BYTES));
 
     // K slice of this CTA (whole cells of 256*kp k); quotients and remainders come from the host
     const int by = blockIdx.y, bx = blockIdx.x, nb = gridDim.x;
@@ -894,22 +900,14 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         }
     }
     for (int i = threadIdx.x; i < p.nxb; i += blockDim.x) mbar_init(smem_u32(xbars + i), blockDim.x);
-    for (int i = threadIdx.x; i < p.nhand; i += blockDim.x) mbar_init(smem_u32(hbars + i), 1);
+    for (int i = threadIdx.x; i <= p.nhand; i += blockDim.x) mbar_init(smem_u32(hbars + i), 1);
     if (threadIdx.x == 0) mbar_fence_init();
     __syncthreads();
 
-    // a blob that was not repacked for this (N, K, KP, ABI version) must not produce plausible numbers: one thread
-    // per CTA checks the header; the flag is published by its first staging-barrier arrival
-    uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
-    const bool checker = (threadIdx.x == W * 32);
-    if (checker) hdr = __ldg(reinterpret_cast<const uint4*>(p.blob - BLOB_HEADER_BYTES));
     // the weight stream is under way; everything below touches data of the previous kernel
     pdl_wait();
     pdl_launch_dependents();
     if (threadIdx.x == 0) NVFP4_TRACE(2);
-    if (checker)
-        *blob_flag = (hdr.x == p.hdr_expect.x) && (hdr.y == p.hdr_expect.y) && (hdr.z == p.hdr_expect.z) &&
-                     (hdr.w == p.hdr_expect.w);
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
     const float gx_raw = (MODE == KMODE_W4A16 || fused || p.gscale_per_row) ? 1.0f : __ldg(p.x_gscale);
@@ -918,6 +916,12 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     else if (fused)          stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
     else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars);
     if (threadIdx.x == W * 32) NVFP4_TRACE(9);
+    const uint32_t hdr_bar = smem_u32(hbars + p.nhand);
+    if (checker) {                                                          // after this thread's share of the staging
+        *blob_flag = (hdr.x == p.hdr_expect.x) && (hdr.y == p.hdr_expect.y) && (hdr.z == p.hdr_expect.z) &&
+                     (hdr.w == p.hdr_expect.w);
+        mbar_arrive(hdr_bar);
+    }
 
     if (!consumer) {                                                        // ---- closer warps ----
         // units this CTA holds only a part of: the (at most two) leftover units, and with K slices every whole unit
@@ -927,6 +931,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
             if (j == 0 && (c.n0 == 0 || (p.ksplit == 1 && c.n0 == ncw))) continue;
             if (j == 1 && c.na - c.n0 == 0) continue;                       // (a second leftover unit is never whole)
             mbar_wait(smem_u32(hbars + j), 0u);
+            mbar_wait(hdr_bar, 0u);
             float g = gw_raw;
             if (MODE != KMODE_W4A16) {
                 g = g * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw);
@@ -967,7 +972,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     uint32_t phase = 0;
     // segments: a leftover cell (phase A) is a segment of its own; in phase B a segment ends with its unit
     int c_ul = 0, seg_left = 0, seg_cell0 = 0, seg_len = 0, a_k = 0;
-    bool seg_first = true, seg_in_a = false, b_started = false;
+    bool seg_first = true, seg_in_a = false, b_started = false, hdr_known = false;
     const uint8_t* xlane = xlane0;
     int x_need = 0;
     int x_have = 0;                                                         // items known to be staged
@@ -1053,7 +1058,8 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
             float gs = gw_raw;
             if (MODE == KMODE_W4A4_I8) gs = (gs * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw)) * 0.25f;   // ints are 2*e
             if (MODE == KMODE_W4A4_H)  gs = gs * (fused ? *reinterpret_cast<volatile float*>(gx_slot) : gx_raw);
-            if (!*blob_flag) gs = __int_as_float(0x7FC00000);               // (published before the first staging barrier)
+            if (!hdr_known) { mbar_wait(hdr_bar, 0u); hdr_known = true; }   // (long complete by now)
+            if (!*blob_flag) gs = __int_as_float(0x7FC00000);
             const int left = total - f - 1;
             if (seg_in_a) {
                 finish_leftover_cell<M, R>(p, c, acc, aslots, hand, hbars, cnt, warp + a_k * W, lane, part, rsub, rpt, gs);

@@ -33,7 +33,7 @@ constexpr int CELL_BYTES  = CELL_CODES + CELL_SCALES;   // 4608 = 0.5625 B per w
 
 // Versioned blob header (the only persistent artefact of the library).  The GEMV
 // compares the first four words with what its launch expects and writes NaN outputs on a mismatch.
-constexpr int      BLOB_HEADER_BYTES = 128;             // keeps the cells 128-byte aligned
+constexpr int      BLOB_HEADER_BYTES = 128;             // keeps the cells 128-byte aligned (512 measured no faster)
 constexpr uint32_t BLOB_MAGIC        = 0x3446564Eu;     // "NVF4"
 struct BlobHeader {
     uint32_t magic;          // BLOB_MAGIC
