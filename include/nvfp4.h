@@ -210,6 +210,30 @@ int nvfp4_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, u
  */
 int nvfp4_silu_mul(const void* gu_bf16, int M, int I, void* h_bf16, void* stream);
 
+/*
+ * The ReSET sampler step (Sec. 4 :107-139, the paper's titular method): for each of B
+ * sequences, one decoding position in ONE launch --
+ *   H_t = entropy of softmax(z_t) (nats, :54)  ->  H_bar (running global mean) and H_step (hybrid step-entropy
+ *   estimator HSE, Eq. 3 :134: mean of the min(w, t+1) most recent H_i while t - t0 < w, else the mean over the
+ *   current step)  ->  tau_t = tau0 if H_step <= H_bar else H_step (SAT, Eq. 2 :113)  ->  T_t = t_low if H_t < tau_t
+ *   else t_high (Eq. 1 :90)  ->  top-p sample from softmax(z_t / T_t): the kept set is every token whose strictly more
+ *   probable mass is < top_p, the draw is the exponential race argmax z_v/T_t - log(-log u_v) with u_v from
+ *   Philox4x32-10 (counter (v, t, 0, 0), key = seed), u = ((x0 >> 9) + 0.5) * 2^-23, ties to the lowest index
+ *   ->  if the sampled token is `delimiter_token` ("\n\n", :367) the next step starts at t + 1.
+ *   logits [device] F32 or BF16 (NVFP4_DTYPE_*), row b at logits + b*ld elements; V <= 163840, ld >= V
+ *   state  [device] B * reset_sampler_state_bytes() bytes, 8-byte aligned, ZERO-FILLED before the first token of a
+ *          sequence; read and updated by every call (ring of the last 32 entropies, sums, t, t0)
+ *   w in 1..32 (paper: 32, :139);  tau0 per model (Table 8 :414-423);  t_low / t_high / top_p as in :139, :412
+ *   token_out [device] int32 [B];  diag_out [device] optional float [B][8]: H_t, H_step, H_bar, tau_t, T_t,
+ *          size of the kept set, t + 1, t0 after the step
+ * Asynchronous on `stream`, graph capturable, deterministic (fixed-order reductions); one thread-block cluster of
+ * 8 CTAs per sequence keeps the vocabulary in registers (the logits are read once).
+ */
+size_t reset_sampler_state_bytes(void);
+int reset_sampler_step(const void* logits, int logits_dtype, int B, int V, int64_t ld, void* state,
+                       float tau0, float t_low, float t_high, float top_p, int w, int delimiter_token,
+                       unsigned long long seed, int* token_out, float* diag_out, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

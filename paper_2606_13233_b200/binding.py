@@ -25,7 +25,8 @@ ERR_NAMES = {0: "NVFP4_OK", -1: "NVFP4_ERR_INVALID_ARG", -2: "NVFP4_ERR_UNSUPPOR
 SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp4_repacked_bytes",
            "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
            "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant",
-           "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts", "nvfp4_silu_mul_quantize")
+           "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts", "nvfp4_silu_mul_quantize",
+           "reset_sampler_state_bytes", "reset_sampler_step")
 
 
 class Nvfp4Error(RuntimeError):
@@ -71,6 +72,11 @@ def _load():
     lib.nvfp4_gemv_get_config.argtypes = [c_int, c_int, c_int, c_int] + [ctypes.POINTER(c_int)] * 6
     lib.nvfp4_silu_mul_quantize.restype = c_int
     lib.nvfp4_silu_mul_quantize.argtypes = [vp, c_int, c_int, vp, vp, vp, c_int, vp, vp]
+    lib.reset_sampler_state_bytes.restype = c_sz
+    lib.reset_sampler_state_bytes.argtypes = []
+    lib.reset_sampler_step.restype = c_int
+    lib.reset_sampler_step.argtypes = [vp, c_int, c_int, c_int, c_i64, vp, ctypes.c_float, ctypes.c_float, ctypes.c_float,
+                                       ctypes.c_float, c_int, c_int, ctypes.c_uint64, vp, vp, vp]
     lib.nvfp4_silu_mul.restype = c_int
     lib.nvfp4_silu_mul.argtypes = [vp, c_int, c_int, vp, vp]
     return lib
@@ -220,3 +226,20 @@ def nvfp4_silu_mul(gu_bf16, h=None):
         h = torch.empty((M, I), dtype=torch.bfloat16, device=gu_bf16.device)
     _check(lib.nvfp4_silu_mul(_ptr(gu_bf16), M, I, _ptr(h), _stream()))
     return h
+
+
+def reset_sampler_new_state(B=1, device="cuda"):
+    """zero-filled ReSET state for B sequences."""
+    return torch.zeros(B * lib.reset_sampler_state_bytes(), dtype=torch.uint8, device=device)
+
+
+def reset_sampler_step(logits, state, tau0, t_low, t_high, top_p=0.95, w=32, delimiter_token=-1, seed=0,
+                       token_out=None, diag_out=None):
+    """one ReSET decoding step for every row of logits [B, V] (float32 or bfloat16).  Returns (tokens int32 [B], diag)."""
+    Bn, V = logits.shape
+    if token_out is None:
+        token_out = torch.empty(Bn, dtype=torch.int32, device=logits.device)
+    dt = DTYPE_F32 if logits.dtype == torch.float32 else DTYPE_BF16
+    _check(lib.reset_sampler_step(_ptr(logits), dt, Bn, V, logits.stride(0), _ptr(state), tau0, t_low, t_high, top_p, w,
+                                  delimiter_token, seed, _ptr(token_out), _ptr(diag_out), _stream()))
+    return token_out, diag_out

@@ -197,6 +197,22 @@ int nvfp4_gemv_get_config(int mode, int M, int N, int K, int* ksplit, int* warps
     return NVFP4_OK;
 }
 
+size_t reset_sampler_state_bytes(void) { return RESET_STATE_BYTES; }
+
+int reset_sampler_step(const void* logits, int logits_dtype, int B, int V, int64_t ld, void* state, float tau0, float t_low,
+                       float t_high, float top_p, int w, int delimiter_token, unsigned long long seed, int* token_out,
+                       float* diag_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!logits || !state || !token_out) return NVFP4_ERR_INVALID_ARG;
+    if (logits_dtype != NVFP4_DTYPE_F32 && logits_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (!(t_low > 0.0f) || !(t_high > 0.0f) || !(top_p > 0.0f) || top_p > 1.0f || w < 1 || w > 32) return NVFP4_ERR_INVALID_ARG;
+    if (B < 1 || B > 1024 || V < 1 || V > 163840 || ld < V) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if ((reinterpret_cast<uintptr_t>(state) & 7u) || (reinterpret_cast<uintptr_t>(logits) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_reset_sampler(logits, logits_dtype == NVFP4_DTYPE_BF16, B, V, ld, state, tau0, t_low, t_high, top_p,
+                                         w, delimiter_token, seed, token_out, diag_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 /* debug hook (not declared in include/nvfp4.h): device buffer of 16 x u64 per CTA that the GEMV fills with
  * %globaltimer stamps of its phases; NULL switches tracing off. */
 int nvfp4_debug_set_trace(void* device_buffer) {

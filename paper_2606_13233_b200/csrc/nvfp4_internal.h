@@ -64,4 +64,9 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
 
 cudaError_t launch_silu_mul(const void* gu, int M, int I, void* h, cudaStream_t st);
 
+constexpr int RESET_STATE_BYTES = 160;
+cudaError_t launch_reset_sampler(const void* logits, int logits_bf16, int B, int V, int64_t ld, void* state, float tau0,
+                                 float t_low, float t_high, float top_p, int w, int delimiter, unsigned long long seed,
+                                 int* token_out, float* diag_out, cudaStream_t st);
+
 }  // namespace nvfp4

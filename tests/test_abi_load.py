@@ -19,7 +19,7 @@ def lib():
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "nvfp4.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(nvfp4_[a-z0-9_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b((?:nvfp4|reset_sampler)_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_symbols_exported(lib):
