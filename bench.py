@@ -395,6 +395,32 @@ def chain_ms_per_token(M, layers, peak):
             "floor_ms_at_peak": round(wb / peak / 1e6, 3)}
 
 
+def sampler_us_per_token(V=151936):
+    """the ReSET sampler step (reset_sampler_step, Sec. 4) on a Qwen3-sized vocabulary: us per decoded token,
+    CUDA-graph replay over 64 distinct logit rows (cold-ish: 39 MB), B = 1 and B = 8 sequences per launch."""
+    import torch
+    from paper_2606_13233_b200 import binding as B
+    out = {"vocab": V, "paper_us_per_token": 100.0, "paper_ref": "PAPER.md:267 (~100 us per token on Qwen3-32B, context)"}
+    gen = torch.Generator(device="cuda"); gen.manual_seed(1)
+    for nb in (1, 8):
+        rows = 64
+        z = torch.randn((rows, nb, V), device="cuda", dtype=torch.float32, generator=gen) * 1.5
+        z[:, :, :6] += 10.0
+        st = B.reset_sampler_new_state(nb)
+        tok = torch.empty(nb, dtype=torch.int32, device="cuda")
+        B.reset_sampler_step(z[0], st, 0.5363, 0.3, 1.0, token_out=tok)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for r in range(rows):
+                B.reset_sampler_step(z[r], st, 0.5363, 0.3, 1.0, 0.95, 32, 198, 7, token_out=tok)
+        us = time_graph(torch, g, 10, 3) / rows * 1e3
+        out[f"us_per_token_b{nb}"] = round(us, 2)
+        del g, z
+    out["algorithmic_bytes_per_token"] = V * 4
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -466,7 +492,7 @@ def run_ours(args):
     del wl
     torch.cuda.empty_cache()
 
-    per_m, chain, roofline_alu = {}, None, None
+    per_m, chain, roofline_alu, sampler = {}, None, None, None
     if rank == 0 and not args.headline_only:
         # ---- the whole metric: the step at M = 1, 2, 4, 8; per shape W4A4 / W4A16 / cuBLAS BF16, cold L2 --------
         for m in MS:
@@ -510,6 +536,7 @@ def run_ours(args):
                         "how": "achieved = (8M dp4a + 3M packed FP32)/32 heavy-pipe lane-instructions per weight x weights/s at "
                                "M = 8; peak = 64 lanes/clk/SM (measured, profiles/r02_microbench.md) x 148 SMs x sampled SM clock",
                         "hbm_frac_same_kernels": per_m["8"]["gemv_only_frac"]}
+        sampler = sampler_us_per_token()
         if not args.no_chain:
             try:
                 chain = chain_ms_per_token(1, args.layers, peak)
@@ -539,6 +566,7 @@ def run_ours(args):
                            "ms_per_step": ms_fused, "value": job_value(b_step, world, ms_fused), "unit": UNIT},
             "per_m": per_m,
             "chain": chain,
+            "sampler": sampler,
             "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone)",
                          "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": ach / peak,
                          "traffic": TRAFFIC_BYTES_PER_STEP.get(M),
@@ -560,7 +588,7 @@ def run_ours(args):
 
 # per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from the committed
 # `ncu --set full` capture of the same kernels; a constant taken from that file, NOT produced by this run.
-TRAFFIC_BYTES_PER_STEP = {1: 279.68e6}
+TRAFFIC_BYTES_PER_STEP = {1: 280.11e6}
 TRAFFIC_SOURCE = ("constant from profiles/r02_ncu_full_m1.md (ncu --set full capture of the 4 GEMV launches of this step; "
                   "algorithmic: 274.4 MB); not measured by this run")
 
