@@ -142,6 +142,20 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
                void* workspace, size_t ws_bytes, void* stream);
 
 /*
+ * Any-M entry point (the paper's runtime dispatches per (M, shape) between its CUDA-core kernel and a tensor-core GEMM,
+ * PAPER.md:526-532 App. C.3; this library has only the CUDA-core kernel): M <= 8 is nvfp4_gemv; larger M runs as
+ * ceil(M/8) consecutive GEMV passes over 8-row chunks of x / y on the same stream (W is streamed once per chunk:
+ * correct and deterministic, but not a prefill kernel).  x_scales is [M, K/16] contiguous, x_gscale one float for
+ * the whole [M, K] tensor; rows must be 16-byte aligned (ldx % 16 == 0 for codes, ldx % 8 == 0 for BF16; ldy * element size % 16 == 0).
+ * workspace >= nvfp4_linear_workspace_bytes(M, N, K), zero-filled once.
+ */
+size_t nvfp4_linear_workspace_bytes(int M, int N, int K);
+int nvfp4_linear(int mode, const void* w_blob, const float* w_gscale, int N, int K,
+                 const void* x, const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx,
+                 void* y, int y_dtype, int64_t ldy,
+                 void* workspace, size_t ws_bytes, void* stream);
+
+/*
  * Per-token (row-wise) activation global scales (R3): the same W4A4 GEMV
  * with x_gscales = M floats, row m of Y scaled by w_gscale * x_gscales[m].  Feed it from
  * nvfp4_quantize_act(..., NVFP4_GSCALE_DYNAMIC_PER_ROW): a row's codes then no longer depend on the other

@@ -26,7 +26,7 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
            "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant",
            "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts", "nvfp4_silu_mul_quantize",
-           "reset_sampler_state_bytes", "reset_sampler_step")
+           "reset_sampler_state_bytes", "reset_sampler_step", "nvfp4_linear", "nvfp4_linear_workspace_bytes")
 
 
 class Nvfp4Error(RuntimeError):
@@ -58,6 +58,10 @@ def _load():
     lib.nvfp4_gemv.restype = c_int
     lib.nvfp4_gemv.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64,
                                vp, c_sz, vp]
+    lib.nvfp4_linear_workspace_bytes.restype = c_sz
+    lib.nvfp4_linear_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_linear.restype = c_int
+    lib.nvfp4_linear.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_rowscale.restype = c_int
     lib.nvfp4_gemv_rowscale.argtypes = [vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_set_layout_kparts.restype = c_int
@@ -155,6 +159,18 @@ def nvfp4_gemv(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, y=
         workspace = new_workspace(M, N, K, x.device)
     _check(lib.nvfp4_gemv(mode, _ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x), _ptr(x_scales), _ptr(x_gscale), M,
                           x.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
+    return y
+
+
+def nvfp4_linear(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, y=None, y_dtype=DTYPE_BF16, workspace=None):
+    """any M: ceil(M/8) GEMV passes over 8-row chunks (see include/nvfp4.h)."""
+    M = x.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x.device)
+    if workspace is None:
+        workspace = torch.zeros(max(16, lib.nvfp4_linear_workspace_bytes(M, N, K)), dtype=torch.uint8, device=x.device)
+    _check(lib.nvfp4_linear(mode, _ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x), _ptr(x_scales), _ptr(x_gscale), M,
+                            x.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
     return y
 
 

@@ -136,6 +136,34 @@ int nvfp4_gemv(int mode, const void* w_blob, const float* w_gscale, int N, int K
                        ws_bytes, stream);
 }
 
+size_t nvfp4_linear_workspace_bytes(int M, int N, int K) {
+    if (M < 1 || !shape_ok(1, N, K)) return 0;
+    const size_t a = nvfp4_gemv_workspace_bytes(M < 8 ? M : 8, N, K);
+    const size_t b = (M > 8 && (M % 8) != 0) ? nvfp4_gemv_workspace_bytes(M % 8, N, K) : 0;
+    return a > b ? a : b;
+}
+
+int nvfp4_linear(int mode, const void* w_blob, const float* w_gscale, int N, int K, const void* x,
+                 const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx, void* y, int y_dtype,
+                 int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+    if (M < 1 || M > (1 << 20)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (mode != NVFP4_MODE_W4A4 && mode != NVFP4_MODE_W4A16) return NVFP4_ERR_INVALID_ARG;
+    if (!x || !y) return NVFP4_ERR_INVALID_ARG;
+    // dispatch rule (App. C.3 dispatches per (M, shape) between the CUDA-core kernel and a tensor-core GEMM):
+    // this library has only the CUDA-core kernel, so any M runs as ceil(M/8) passes of it over 8-row chunks
+    const size_t xrow = (mode == NVFP4_MODE_W4A4) ? (size_t)ldx : (size_t)ldx * 2;
+    const size_t yrow = (size_t)ldy * (y_dtype == NVFP4_DTYPE_F32 ? 4 : 2);
+    for (int r = 0; r < M; r += 8) {
+        const int m = (M - r) < 8 ? (M - r) : 8;
+        const int rc = gemv_common(mode, w_blob, w_gscale, N, K, static_cast<const uint8_t*>(x) + (size_t)r * xrow,
+                                   x_scales ? x_scales + (size_t)r * (K / 16) : nullptr, x_gscale, 0, m, ldx,
+                                   static_cast<uint8_t*>(y) + (size_t)r * yrow, y_dtype, ldy, workspace, ws_bytes, stream);
+        if (rc != NVFP4_OK) return rc;
+    }
+    return NVFP4_OK;
+}
+
 int nvfp4_gemv_rowscale(const void* w_blob, const float* w_gscale, int N, int K, const void* x_codes,
                         const uint8_t* x_scales, const float* x_gscales, int M, int64_t ldx, void* y, int y_dtype,
                         int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {

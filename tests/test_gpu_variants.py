@@ -182,3 +182,25 @@ def test_table4_shapes_sampled_rows(B, name, N, K, M):
     if M == 1:
         yf = B.nvfp4_gemv_fused_quant(blob, U.dev_f32(gw), N, K, U.dev_bf16_from_bits(xbits), y_dtype=B.DTYPE_BF16)
         assert torch.equal(yf, y)
+
+
+# ---- any-M entry point (dispatch rule) --------------------------------------------------------
+@pytest.mark.parametrize("M", [9, 20, 64])
+def test_linear_any_m(B, M):
+    N, K = 1000, 2576
+    wc, ws, gw = U.oracle_weight(N, K, 9, 3)
+    blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws))
+    rng = np.random.default_rng(M)
+    xf = (rng.standard_normal((M, K)) * rng.choice([0.5, 1.0, 4.0], size=(M, 1))).astype(np.float32)
+    xbits = orc.f32_to_bf16_bits(xf)
+    oxc, oxs, ogx = orc.quantize(orc.bf16_bits_to_f32(xbits))               # one global scale for the whole [M, K]
+    Y, A = orc.gemv_w4a4(wc, ws, gw, oxc, oxs, ogx)
+    y = B.nvfp4_linear(B.MODE_W4A4, blob, U.dev_f32(gw), N, K, U.dev_u8(oxc), U.dev_u8(oxs), U.dev_f32(ogx), y_dtype=B.DTYPE_F32)
+    torch.cuda.synchronize()
+    U.check_gemv(U.host_y_f64(y), Y, A, f"linear w4a4 M={M}")
+    y16 = B.nvfp4_linear(B.MODE_W4A16, blob, U.dev_f32(gw), N, K, U.dev_bf16_from_bits(xbits), y_dtype=B.DTYPE_BF16)
+    Y2, A2 = orc.gemv_w4a16(wc, ws, gw, orc.bf16_bits_to_f32(xbits))
+    U.check_gemv(U.host_y_f64(y16), Y2, A2, f"linear w4a16 M={M}")
+    # chunks reproduce the 8-row GEMV exactly
+    y8 = B.nvfp4_gemv(B.MODE_W4A4, blob, U.dev_f32(gw), N, K, U.dev_u8(oxc[:8]), U.dev_u8(oxs[:8]), U.dev_f32(ogx), y_dtype=B.DTYPE_F32)
+    assert torch.equal(y[:8], y8)
