@@ -124,8 +124,9 @@ GemvConfig gemv_pick_config(int mode, int M, int N, int K, int kp) {
     GemvConfig c;
     const int kmode = gemv_kmode(mode, M);
     const bool big = (long long)N * K >= (128ll << 20);                   // gate_up-sized weights: 16 warps pay (M <= 2)
+    const bool mid = (long long)N * K >= (120ll << 20);                   // down-sized: 16 warps pay at M = 1 (profiles/r02_sweep.md)
     c.rows = 1;
-    c.warps = (kmode == KMODE_W4A16 || M >= 3) ? 12 : (big ? 16 : 12);
+    c.warps = (kmode == KMODE_W4A16 || M >= 3) ? 12 : ((big || (mid && M == 1)) ? 16 : 12);
     c.stages = 2;        // three stages measured 3-5 % slower everywhere: more bytes in flight than the memory system wants
     c.ksplit = 1;
     c.cps = 1;           // two half-size CTAs per SM measured no faster
@@ -175,6 +176,13 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     p.base = P.base; p.ur = P.ur; p.whole_units = P.whole;
     for (int v = 0; v < 2; ++v) { p.nba[v] = P.nba[v]; p.a_q[v] = P.a_q[v]; p.a_r[v] = P.a_r[v]; p.inv_a[v] = P.inv_a[v]; }
     p.amax = P.amax; p.jmax = P.jmax; p.nxb = P.nxb; p.nhand = P.nhand;
+    p.fd_w = fastdiv_make((uint32_t)P.W);
+    for (int v = 0; v < 2; ++v) { p.fd_ncw[v] = fastdiv_make((uint32_t)(P.cells_q + v)); p.fd_nba[v] = fastdiv_make((uint32_t)P.nba[v]); }
+    {
+        const uint32_t mm[13] = {P.map.xs, P.map.ring, P.map.slots, P.map.aslots, P.map.hand, P.map.bars, P.map.xbars, P.map.hbars,
+                                 P.map.cnt, P.map.bstart, P.map.astart, P.map.misc, P.map.total};
+        for (int i = 0; i < 13; ++i) p.smem_map[i] = mm[i];
+    }
     p.y_bf16 = (y_dtype == NVFP4_DTYPE_BF16);
     p.zero = 0;
     p.fuse_quant = fuse_quant ? 1 : 0;

@@ -56,6 +56,7 @@ struct GemvParams {
     int base, ur;
     int whole_units;               // 1: no leftover stream; the first `ur` CTAs own base + 1 whole units instead
     int nba[2], a_q[2], a_r[2];
+    FastDiv fd_w, fd_ncw[2], fd_nba[2];   // divisors: consumer warps, cells per unit (per variant), phase-A CTAs (per variant)
     float inv_a[2];                // nba / (ur*ncw_v): estimate for the inverse of the share start
     int amax;                      // max leftover cells per CTA
     int jmax;                      // max number of CTAs of one slice that share a leftover unit
@@ -67,6 +68,7 @@ struct GemvParams {
     int gscale_per_row;            // x_gscale holds M per-row (per-token) global scales
     float* x_gscale_out;           // fuse_quant: optional device float that receives the activation global scale
     uint4 hdr_expect;              // blob_header_words(N, K, kp)
+    uint32_t smem_map[13];         // gemv_smem_map(...) computed by the host (same order as struct SmemMap)
     unsigned long long* trace;     // debug only (nvfp4_debug_set_trace): 16 timestamps per CTA, else NULL
 };
 
@@ -181,9 +183,10 @@ __device__ __forceinline__ void decode_x_block_h(uint2 cw, float sx, uint8_t* ba
     *reinterpret_cast<float*>(base + 64 + half * 4) = sx;
 }
 
-template <int M, bool HALF>
+// `between` runs once, right after the first batch's loads have been issued (their L2 latency hides it)
+template <int M, bool HALF, typename Between>
 __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
-                                             uint64_t* xbars) {
+                                             uint64_t* xbars, Between&& between) {
     const int nblk = ncw * 2 * CELL_VECS * p.kp;                 // 16-blocks in the range
     const int kb_total = p.K >> 4;
     const int kb0 = c0 * 2 * CELL_VECS * p.kp;
@@ -203,6 +206,7 @@ __device__ __forceinline__ void stage_x_w4a4(const GemvParams& p, uint8_t* xs, i
                 sb[t] = __ldg(p.x_scales + (int64_t)m * kb_total + kb0 + blk);
             }
         }
+        if (batch == 0) between();
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
             const int i = base + t * nthr + tid;
@@ -286,9 +290,9 @@ __device__ __forceinline__ void stage_x_fused(const GemvParams& p, uint8_t* xs, 
 }
 
 // W4A16: work item i -> (8-element vector = i / M, m = i % M); progress published in 16-blocks
-template <int M>
+template <int M, typename Between>
 __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, int c0, int ncw, int tid, int nthr,
-                                              uint64_t* xbars) {
+                                              uint64_t* xbars, Between&& between) {
     const int nvec = ncw * 4 * CELL_VECS * p.kp;                 // 8-element vectors per row in the range
     const uint16_t* xb = static_cast<const uint16_t*>(p.x);
     const int total = nvec * M;
@@ -303,6 +307,7 @@ __device__ __forceinline__ void stage_x_w4a16(const GemvParams& p, uint8_t* xs, 
             if (i < total && k_base + v * 8 < p.K)
                 raw[t] = __ldg(reinterpret_cast<const uint4*>(xb + (int64_t)m * p.ldx + k_base + v * 8));
         }
+        if (batch == 0) between();
 #pragma unroll
         for (int t = 0; t < STAGE_BATCH; ++t) {
             const int i = base + t * nthr + tid;
@@ -557,8 +562,15 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
 }
 #ifdef NVFP4_ENABLE_TRACE      // debug builds only (-DNVFP4_ENABLE_TRACE): per-phase %globaltimer stamps, 64 per CTA
 #define NVFP4_TRACE(slot) do { if (p.trace) p.trace[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 64 + (slot)] = globaltimer_ns(); } while (0)
+#define NVFP4_CLK(i) do { if (threadIdx.x == 0) clk_[i] = clock64(); } while (0)
+#define NVFP4_CLK_DECL long long clk_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
+#define NVFP4_CLK_FLUSH do { if (threadIdx.x == 0 && p.trace) for (int i_ = 0; i_ < 16; ++i_) \
+    p.trace[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 64 + 48 + i_] = (unsigned long long)(clk_[i_] ? clk_[i_] - clk_[0] : 0); } while (0)
 #else
 #define NVFP4_TRACE(slot) do { } while (0)
+#define NVFP4_CLK(i) do { } while (0)
+#define NVFP4_CLK_DECL do { } while (0)
+#define NVFP4_CLK_FLUSH do { } while (0)
 #endif
 
 __device__ __forceinline__ void store_y(const GemvParams& p, int m, int n, float v) {
@@ -768,11 +780,14 @@ __host__ __device__ constexpr int gemv_max_threads(int kmode, int M, int R) {
 template <int MODE, int M, int R>
 __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(const GemvParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
+    NVFP4_CLK_DECL;
+    NVFP4_CLK(0);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = p.warps, S = p.stages;
     const int rsub = lane & ((32 >> p.kp_shift) - 1), part = lane >> (5 - p.kp_shift);   // lane = part*rpt + rsub
     const int rpt = 32 >> p.kp_shift;
     constexpr uint32_t STAGE_BYTES = R * CELL_BYTES;
+    NVFP4_CLK(1);
     if (threadIdx.x == 0) NVFP4_TRACE(0);
     // a blob that was not repacked for this (N, K, KP, ABI version) must not produce plausible numbers: one thread
     // per CTA (the first stager thread) loads the header right away (a cold DRAM access, kept OFF the staging path)
@@ -795,19 +810,25 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         const unsigned nba = (unsigned)p.nba[c.var], aq = (unsigned)p.a_q[c.var], ar = (unsigned)p.a_r[c.var];
         unsigned a0 = 0, a1 = 0;
         if ((unsigned)bx < nba) {
-            a0 = (unsigned)bx * aq + ((unsigned)bx * ar) / nba;
-            a1 = (unsigned)(bx + 1) * aq + ((unsigned)(bx + 1) * ar) / nba;
+            a0 = (unsigned)bx * aq + fastdiv((unsigned)bx * ar, p.fd_nba[c.var]);
+            a1 = (unsigned)(bx + 1) * aq + fastdiv((unsigned)(bx + 1) * ar, p.fd_nba[c.var]);
         }
         c.a0 = (int)a0; c.na = (int)(a1 - a0);
-        c.qa0 = (int)(a0 / (unsigned)ncw);
+        c.qa0 = (int)fastdiv(a0, p.fd_ncw[c.var]);
         const int room = (c.qa0 + 1) * ncw - c.a0;                          // cells left in the first leftover unit
         c.n0 = c.na < room ? c.na : room;
     }
+    NVFP4_CLK(2);
     const int my_base = p.base + ((p.whole_units && bx < p.ur) ? 1 : 0);   // whole units of this CTA ...
     c.unit0 = bx * p.base + (p.whole_units ? (bx < p.ur ? bx : p.ur) : 0);  // ... starting at this global unit
     const int Bc = my_base * ncw;                                           // phase B cells of this CTA
 
-    const SmemMap map = gemv_smem_map(MODE, M, R, W, S, rpt, ncw_max, p.kp, p.nxb, p.base, nb, p.amax, p.nhand);
+    SmemMap map;                                                            // computed by the host (gemv_smem_map)
+    map.xs = p.smem_map[0]; map.ring = p.smem_map[1]; map.slots = p.smem_map[2]; map.aslots = p.smem_map[3];
+    map.hand = p.smem_map[4]; map.bars = p.smem_map[5]; map.xbars = p.smem_map[6]; map.hbars = p.smem_map[7];
+    map.cnt = p.smem_map[8]; map.bstart = p.smem_map[9]; map.astart = p.smem_map[10]; map.misc = p.smem_map[11];
+    map.total = p.smem_map[12];
+    (void)ncw_max;
     uint8_t* xs = smem + map.xs;                                             // activations
     constexpr int XVS = xvec_stride(MODE, M);
     uint8_t* ring_all = smem + map.ring;
@@ -830,9 +851,9 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     // ---- consumer warps: request the first weight cells before anything else (private ring, private barriers) ----
     // warp w: phase A cells i = w, w + W, ... < na (na_w of them), then phase B cells [bs, be) of the CTA's Bc
     const bool consumer = warp < W;
-    const int na_w = consumer ? (c.na + W - 1 - warp) / W : 0;
-    const int bs = consumer ? Bc - (int)(((unsigned)(W - warp) * (unsigned)Bc) / (unsigned)W) : 0;
-    const int be = consumer ? Bc - (int)(((unsigned)(W - warp - 1) * (unsigned)Bc) / (unsigned)W) : 0;
+    const int na_w = consumer ? (int)fastdiv((unsigned)(c.na + W - 1 - warp), p.fd_w) : 0;
+    const int bs = consumer ? Bc - (int)fastdiv((unsigned)(W - warp) * (unsigned)Bc, p.fd_w) : 0;
+    const int be = consumer ? Bc - (int)fastdiv((unsigned)(W - warp - 1) * (unsigned)Bc, p.fd_w) : 0;
     const int total = na_w + (be - bs);
     const int64_t tile_stride = (int64_t)p.nch * CELL_BYTES;
     uint8_t* ring = ring_all + (size_t)(consumer ? warp : 0) * S * STAGE_BYTES;
@@ -840,7 +861,7 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     const bool leader = consumer && (lane == 0);
     // producer cursor (used by lane 0 only): next cell to request.  The warp's cells form RUNS of cells that are
     // contiguous in the blob: every leftover cell is a run of one, then one run per whole unit touched.
-    int p_left = 0, p_count = 0, p_nv = 0, p_a = 0;
+    int p_left = 0, p_count = 0, p_nv = 0, p_a = 0, p_tile0 = 0;
     bool p_b_started = false;
     uint32_t p_dst = smem_u32(ring), p_bar = smem_u32(bars);
     const uint32_t ring_end = p_dst + (uint32_t)S * STAGE_BYTES;
@@ -850,22 +871,23 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         int tile0;
         if (p_a < na_w) {                                                   // phase A: leftover cell i = warp + p_a*W
             const int fa = c.a0 + warp + p_a * W;
-            const int q = (int)((unsigned)fa / (unsigned)ncw), cell = fa - q * ncw;
+            const int q = (int)fastdiv((unsigned)fa, p.fd_ncw[c.var]), cell = fa - q * ncw;
             tile0 = (p.base * nb + q) * R;
             p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
             p_left = 1;
             ++p_a;
         } else if (!p_b_started) {                                          // phase B starts: cell bs of the CTA's whole units
             p_b_started = true;
-            const int ul = (int)((unsigned)bs / (unsigned)ncw), cell = bs - ul * ncw;
+            const int ul = (int)fastdiv((unsigned)bs, p.fd_ncw[c.var]), cell = bs - ul * ncw;
             tile0 = (c.unit0 + ul) * R;
             p_src = p.blob + ((int64_t)tile0 * p.nch + c0 + cell) * CELL_BYTES;
             p_left = ncw - cell;
         } else {                                                            // next whole unit of the run
             p_src += unit_jump;
             p_left = ncw;
-            tile0 = (int)((p_src - p.blob) / tile_stride);
+            tile0 = p_tile0 + R;
         }
+        p_tile0 = tile0;
         p_nv = p.ntiles - tile0; p_nv = p_nv > R ? R : p_nv;
     };
     auto issue = [&]() {
@@ -879,42 +901,67 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         p_dst += STAGE_BYTES; p_bar += 8;
         if (p_dst == ring_end) { p_dst -= (uint32_t)S * STAGE_BYTES; p_bar -= (uint32_t)S * 8; }
     };
+    NVFP4_CLK(3);
     if (leader) {
         for (int s = 0; s < S; ++s) mbar_init(smem_u32(bars + s), 1);
         mbar_fence_init();
+        NVFP4_CLK(4);
         if (total > 0) next_run();
-        const int npre = total < S ? total : S;
-        for (int i = 0; i < npre; ++i) issue();
+        NVFP4_CLK(5);
+        // ONE cell per warp now: a burst of S cells per warp arrives interleaved (every cell lands at the END of the
+        // burst) and the activation loads issued after griddepcontrol.wait would queue behind all of it
+        if (total > 0) issue();
     }
+    NVFP4_CLK(6);
     if (threadIdx.x == 0) NVFP4_TRACE(1);
 
-    // ---- CTA-wide tables and barriers ----
-    for (int i = threadIdx.x; i < p.base + 3; i += blockDim.x) cnt[i] = 0;
-    if (threadIdx.x <= W) bstart[threadIdx.x] = Bc - (int)(((unsigned)(W - threadIdx.x) * (unsigned)Bc) / (unsigned)W);
-    for (unsigned b = threadIdx.x; b <= (unsigned)nb; b += blockDim.x) {
-#pragma unroll
-        for (int v = 0; v < 2; ++v) {
-            const unsigned nba = (unsigned)p.nba[v];
-            const unsigned bb = b < nba ? b : nba;                          // CTAs that take no part repeat the end
-            astart[v * (nb + 1) + b] = nba ? (int)(bb * (unsigned)p.a_q[v] + (bb * (unsigned)p.a_r[v]) / nba) : 0;
-        }
-    }
+    // ---- CTA-wide barriers (the tables follow under the latency of the activation loads: `deferred` below) ----
     for (int i = threadIdx.x; i < p.nxb; i += blockDim.x) mbar_init(smem_u32(xbars + i), blockDim.x);
     for (int i = threadIdx.x; i <= p.nhand; i += blockDim.x) mbar_init(smem_u32(hbars + i), 1);
     if (threadIdx.x == 0) mbar_fence_init();
+    NVFP4_CLK(7);
     __syncthreads();
+    NVFP4_CLK(8);
 
     // the weight stream is under way; everything below touches data of the previous kernel
     pdl_wait();
     pdl_launch_dependents();
+    NVFP4_CLK(9);
     if (threadIdx.x == 0) NVFP4_TRACE(2);
     // global scales: issue the loads now, combine them only when the first segment is written
     const float gw_raw = __ldg(p.w_gscale);
     const float gx_raw = (MODE == KMODE_W4A16 || fused || p.gscale_per_row) ? 1.0f : __ldg(p.x_gscale);
+    // Runs in every thread right after its first activation loads are in flight (or before the fused quantizer):
+    // the rest of the ring prefetch, then the CTA-wide tables.  Every thread's stores precede its arrival on the first
+    // staging barrier, and every reader has waited on a staging barrier (or on a hand-off that follows one).
+    bool deferred_done = false;
+    auto deferred = [&]() {
+        deferred_done = true;
+        if (leader) {
+            const int npre = total < S ? total : S;
+            while (p_count < npre) issue();
+        }
+        for (int i = threadIdx.x; i < p.base + 3; i += blockDim.x) cnt[i] = 0;
+        if (threadIdx.x <= W) bstart[threadIdx.x] = Bc - (int)fastdiv((unsigned)(W - threadIdx.x) * (unsigned)Bc, p.fd_w);
+        if (p.nba[0] | p.nba[1]) {
+            for (unsigned b = threadIdx.x; b <= (unsigned)nb; b += blockDim.x) {
+#pragma unroll
+                for (int v = 0; v < 2; ++v) {
+                    const unsigned nba = (unsigned)p.nba[v];
+                    const unsigned bb = b < nba ? b : nba;                  // CTAs that take no part repeat the end
+                    astart[v * (nb + 1) + b] = nba ? (int)(bb * (unsigned)p.a_q[v] + fastdiv(bb * (unsigned)p.a_r[v], p.fd_nba[v])) : 0;
+                }
+            }
+        }
+    };
     // activation staging: every thread of the CTA takes its share
-    if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars);
-    else if (fused)          stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
-    else                     stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars);
+    if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, deferred);
+    else if (fused) {
+        deferred();
+        stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);
+    } else stage_x_w4a4<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, deferred);
+    if (!deferred_done) deferred();
+    NVFP4_CLK(10);
     if (threadIdx.x == W * 32) NVFP4_TRACE(9);
     const uint32_t hdr_bar = smem_u32(hbars + p.nhand);
     if (checker) {                                                          // after this thread's share of the staging
@@ -981,11 +1028,11 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         int cell;
         if (a_k < na_w) {
             const int fa = c.a0 + warp + a_k * W;
-            cell = fa - (int)((unsigned)fa / (unsigned)ncw) * ncw;
+            cell = fa - (int)fastdiv((unsigned)fa, p.fd_ncw[c.var]) * ncw;
             seg_in_a = true; seg_len = 1;
         } else if (!b_started) {
             b_started = true; seg_in_a = false;
-            c_ul = (int)((unsigned)bs / (unsigned)ncw);
+            c_ul = (int)fastdiv((unsigned)bs, p.fd_ncw[c.var]);
             cell = bs - c_ul * ncw;
             seg_len = ncw - cell < left ? ncw - cell : left;
         } else {
@@ -1000,7 +1047,10 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     for (int f = 0; f < total; ++f) {
         while (x_have < x_need) { mbar_wait(xbar, 0u); xbar += 8; x_have += stage_items; }
         if (threadIdx.x == 0 && f == 0) NVFP4_TRACE(3);
+        if (f == 0) NVFP4_CLK(11);
         mbar_wait(bar, phase);
+        if (f == 0) NVFP4_CLK(12);
+
         if (threadIdx.x == 0 && f < 3) NVFP4_TRACE(4 + f);
         if (lane == 0 && f == 1) NVFP4_TRACE(40 + warp);
 
@@ -1077,6 +1127,8 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
                 for (int m = 0; m < M; ++m) acc[r][m] = 0.0f;
         }
     }
+    NVFP4_CLK(14);
+    NVFP4_CLK_FLUSH;
     if (lane == 0 && (warp == 0 || warp == W - 1)) NVFP4_TRACE(warp == 0 ? 7 : 14);
     if (lane == 0) NVFP4_TRACE(16 + warp);
 }

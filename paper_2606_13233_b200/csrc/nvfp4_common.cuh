@@ -80,6 +80,23 @@ __host__ __device__ inline int layout_kparts(int N, int K) {
     return best;
 }
 
+// ---- division by a launch-constant divisor without the ~25-instruction udiv sequence ----------------------------------
+// q = floor(n / d) for 0 <= n < 2^31:  mul = ceil(2^(31+L) / d), L = ceil(log2 d);  q = (n * mul) >> (31 + L).
+// (n*mul/2^(31+L) = n/d + n*e/2^(31+L) with 0 <= e < 1, and n*e/2^(31+L) < 2^-L <= 1/d: the floor cannot move.)
+struct FastDiv { uint32_t mul; uint32_t sh; };
+__host__ __device__ inline FastDiv fastdiv_make(uint32_t d) {
+    FastDiv f;
+    if (d == 0) d = 1;
+    uint32_t L = 0;
+    while ((1ull << L) < d) ++L;
+    f.mul = (uint32_t)(((1ull << (31 + L)) + d - 1) / d);
+    f.sh = 31 + L;
+    return f;
+}
+__host__ __device__ __forceinline__ uint32_t fastdiv(uint32_t n, const FastDiv& f) {
+    return (uint32_t)(((unsigned long long)n * f.mul) >> f.sh);
+}
+
 // ---- conversions ------------------------------------------------------------------------
 // E4M3 byte pair -> two FP32 (exact): F2FP.E4M3.UNPACK then two f16->f32.
 __device__ __forceinline__ float2 e4m3x2_to_float2(uint16_t v) {
