@@ -248,6 +248,65 @@ int reset_sampler_step(const void* logits, int logits_dtype, int B, int V, int64
                        float tau0, float t_low, float t_high, float top_p, int w, int delimiter_token,
                        unsigned long long seed, int* token_out, float* diag_out, void* stream);
 
+/*
+ * Tensor-core NVFP4 GEMM (App. C.3 :526-532, Table 16 :560-575: the paper dispatches
+ * large M to a tensor-core GEMM).  Y[M,N] = X[M,K] . W[N,K]^T, both operands NVFP4, on tcgen05 block-scaled MMAs
+ * (kind::mxf4nvf4, scale_vec::4X: E2M1 codes and E4M3 block scales go to the tensor core as they are, FP32
+ * accumulation in tensor memory).  The weight tile is the MMA's A operand (128 weight rows) and the tokens are its N
+ * dimension, so W is streamed from HBM once per 128 tokens for ANY M >= 1 (M <= 128: exactly once).
+ *
+ *   nvfp4_gemm_repacked_bytes   size of the tensor-core blob for (N, K); 0 if the shape is unsupported
+ *                               (requires K % 256 == 0, K >= 256, N >= 1).  Same 0.5625 B per weight as the GEMV blob,
+ *                               rows padded to a multiple of 128.
+ *   nvfp4_gemm_repack_weight    canonical codes [N,K/2] + scales [N,K/16] (device) -> blob (device, 128-byte aligned
+ *                               recommended, 16 required): a pure byte permutation into the shared-memory image of
+ *                               the MMA operands (8-row x 16-byte core matrices; scale chunks in tcgen05.cp order)
+ *                               behind a versioned 128-byte header.  Offline, once.  nvfp4_gemm_unpack_weight is its
+ *                               exact inverse.  The blob is NOT interchangeable with nvfp4_repack_weight's: the GEMM
+ *                               writes NaN outputs when handed a blob whose header does not match (N, K).
+ *   nvfp4_gemm                  x_codes [M, K/2] (row stride ldx bytes, ldx % 16 == 0), x_scales [M, K/16] contiguous,
+ *                               x_gscale one device float (gscale_per_row = 0) or M floats (= 1); y F32 or BF16
+ *                               [M, N] (row stride ldy elements).  Launches a small activation re-layout kernel and
+ *                               the GEMM (per 128-token chunk) on `stream`; graph capturable, deterministic
+ *                               (fixed-order stream-K fix-up), programmatic dependent launch.
+ *                               workspace >= nvfp4_gemm_workspace_bytes(M, N, K), 16-byte aligned, zero-filled once
+ *                               before first use (the kernel leaves its counters zero).
+ * Acceptance as for nvfp4_gemv: |y - y_ref| <= 1e-3 * sum_k|w_k x_k| + 1e-6.
+ */
+size_t nvfp4_gemm_repacked_bytes(int N, int K);
+int nvfp4_gemm_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream);
+int nvfp4_gemm_unpack_weight(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, void* stream);
+size_t nvfp4_gemm_workspace_bytes(int M, int N, int K);
+int nvfp4_gemm(const void* w_blob_tc, const float* w_gscale, int N, int K,
+               const void* x_codes, const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, int64_t ldx,
+               void* y, int y_dtype, int64_t ldy,
+               void* workspace, size_t ws_bytes, void* stream);
+
+/*
+ * The same GEMM fed without the re-layout kernel (the decode chain's form: quantizer -> GEMM, two launches per
+ * projection like the GEMV path).  The activations of M <= 128 tokens live in the GEMM's own record layout
+ * ("packed": per 256 k one record of MT*128 code bytes in 8-token x 16-byte core matrices followed by four 512-byte
+ * scale chunks, MT = 8, 16, 32, 64 or 128 >= M), nvfp4_gemm_packed_act_bytes(M, K) bytes, 16-byte aligned; the buffer
+ * need not be initialised (columns of tokens >= M are computed and never stored).
+ *   nvfp4_gemm_pack_act             canonical codes / scales -> packed
+ *   nvfp4_quantize_act_packed       nvfp4_quantize_act writing the packed layout directly: the same binary32 sequence,
+ *                                   so pack_act(quantize_act(x)) == quantize_act_packed(x) byte for byte.  M <= 128 for
+ *                                   NVFP4_GSCALE_DYNAMIC / _STATIC, M <= 8 for _DYNAMIC_PER_ROW.
+ *   nvfp4_silu_mul_quantize_packed  nvfp4_silu_mul_quantize writing the packed layout (M * I <= 524288)
+ *   nvfp4_gemm_packed               the GEMM on packed activations; workspace >= nvfp4_gemm_packed_workspace_bytes,
+ *                                   zero-filled once; other arguments as for nvfp4_gemm
+ */
+size_t nvfp4_gemm_packed_act_bytes(int M, int K);
+int nvfp4_gemm_pack_act(const void* x_codes, const uint8_t* x_scales, int M, int K, int64_t ldx, void* xpack_out, void* stream);
+int nvfp4_quantize_act_packed(const void* x_bf16, int M, int K, int64_t ldx, void* xpack_out, float* gscale, int gscale_mode,
+                              void* stream);
+int nvfp4_silu_mul_quantize_packed(const void* gu_bf16, int M, int I, void* xpack_out, float* gscale, int gscale_mode,
+                                   void* h_bf16_opt, void* stream);
+size_t nvfp4_gemm_packed_workspace_bytes(int M, int N, int K);
+int nvfp4_gemm_packed(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* xpack, const float* x_gscale,
+                      int gscale_per_row, int M, void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes,
+                      void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -26,7 +26,11 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_repack_weight", "nvfp4_unpack_weight", "nvfp4_gemv_workspace_bytes", "nvfp4_gemv",
            "nvfp4_gemv_set_config", "nvfp4_gemv_get_config", "nvfp4_silu_mul", "nvfp4_gemv_fused_quant",
            "nvfp4_gemv_rowscale", "nvfp4_set_layout_kparts", "nvfp4_get_layout_kparts", "nvfp4_silu_mul_quantize",
-           "reset_sampler_state_bytes", "reset_sampler_step", "nvfp4_linear", "nvfp4_linear_workspace_bytes")
+           "reset_sampler_state_bytes", "reset_sampler_step", "nvfp4_linear", "nvfp4_linear_workspace_bytes",
+           "nvfp4_gemm_repacked_bytes", "nvfp4_gemm_repack_weight", "nvfp4_gemm_unpack_weight",
+           "nvfp4_gemm_workspace_bytes", "nvfp4_gemm", "nvfp4_gemm_packed_act_bytes", "nvfp4_gemm_pack_act",
+           "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
+           "nvfp4_gemm_packed")
 
 
 class Nvfp4Error(RuntimeError):
@@ -83,6 +87,28 @@ def _load():
                                        ctypes.c_float, c_int, c_int, ctypes.c_uint64, vp, vp, vp]
     lib.nvfp4_silu_mul.restype = c_int
     lib.nvfp4_silu_mul.argtypes = [vp, c_int, c_int, vp, vp]
+    lib.nvfp4_gemm_repacked_bytes.restype = c_sz
+    lib.nvfp4_gemm_repacked_bytes.argtypes = [c_int, c_int]
+    lib.nvfp4_gemm_repack_weight.restype = c_int
+    lib.nvfp4_gemm_repack_weight.argtypes = [vp, vp, c_int, c_int, vp, vp]
+    lib.nvfp4_gemm_unpack_weight.restype = c_int
+    lib.nvfp4_gemm_unpack_weight.argtypes = [vp, c_int, c_int, vp, vp, vp]
+    lib.nvfp4_gemm_workspace_bytes.restype = c_sz
+    lib.nvfp4_gemm_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemm.restype = c_int
+    lib.nvfp4_gemm.argtypes = [vp, vp, c_int, c_int, vp, vp, vp, c_int, c_int, c_i64, vp, c_int, c_i64, vp, c_sz, vp]
+    lib.nvfp4_gemm_packed_act_bytes.restype = c_sz
+    lib.nvfp4_gemm_packed_act_bytes.argtypes = [c_int, c_int]
+    lib.nvfp4_gemm_pack_act.restype = c_int
+    lib.nvfp4_gemm_pack_act.argtypes = [vp, vp, c_int, c_int, c_i64, vp, vp]
+    lib.nvfp4_quantize_act_packed.restype = c_int
+    lib.nvfp4_quantize_act_packed.argtypes = [vp, c_int, c_int, c_i64, vp, vp, c_int, vp]
+    lib.nvfp4_silu_mul_quantize_packed.restype = c_int
+    lib.nvfp4_silu_mul_quantize_packed.argtypes = [vp, c_int, c_int, vp, vp, c_int, vp, vp]
+    lib.nvfp4_gemm_packed_workspace_bytes.restype = c_sz
+    lib.nvfp4_gemm_packed_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemm_packed.restype = c_int
+    lib.nvfp4_gemm_packed.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, c_int, vp, c_int, c_i64, vp, c_sz, vp]
     return lib
 
 
@@ -171,6 +197,91 @@ def nvfp4_linear(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, 
         workspace = torch.zeros(max(16, lib.nvfp4_linear_workspace_bytes(M, N, K)), dtype=torch.uint8, device=x.device)
     _check(lib.nvfp4_linear(mode, _ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x), _ptr(x_scales), _ptr(x_gscale), M,
                             x.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
+    return y
+
+
+def nvfp4_gemm_repack_weight(codes, scales):
+    """canonical codes u8 [N,K/2] + scales u8 [N,K/16] (device) -> tensor-core blob (u8, device)."""
+    N, K = codes.shape[0], codes.shape[1] * 2
+    nbytes = lib.nvfp4_gemm_repacked_bytes(N, K)
+    if nbytes == 0:
+        raise Nvfp4Error(-2, f"tensor-core GEMM needs K % 256 == 0 (N={N}, K={K})")
+    blob = torch.empty(nbytes, dtype=torch.uint8, device=codes.device)
+    _check(lib.nvfp4_gemm_repack_weight(_ptr(codes), _ptr(scales), N, K, _ptr(blob), _stream()))
+    return blob
+
+
+def nvfp4_gemm_unpack_weight(blob, N, K):
+    codes = torch.zeros((N, K // 2), dtype=torch.uint8, device=blob.device)
+    scales = torch.zeros((N, K // 16), dtype=torch.uint8, device=blob.device)
+    _check(lib.nvfp4_gemm_unpack_weight(_ptr(blob), N, K, _ptr(codes), _ptr(scales), _stream()))
+    return codes, scales
+
+
+def nvfp4_gemm_new_workspace(M, N, K, device):
+    return torch.zeros(max(16, lib.nvfp4_gemm_workspace_bytes(M, N, K)), dtype=torch.uint8, device=device)
+
+
+def nvfp4_gemm(w_blob_tc, w_gscale, N, K, x_codes, x_scales, x_gscale, y=None, y_dtype=DTYPE_BF16, workspace=None,
+               gscale_per_row=False):
+    """tensor-core W4A4 GEMM, any M >= 1: Y[M,N] = X . W^T (see include/nvfp4.h)."""
+    M = x_codes.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x_codes.device)
+    if workspace is None:
+        workspace = nvfp4_gemm_new_workspace(M, N, K, x_codes.device)
+    _check(lib.nvfp4_gemm(_ptr(w_blob_tc), _ptr(w_gscale), N, K, _ptr(x_codes), _ptr(x_scales), _ptr(x_gscale),
+                          1 if gscale_per_row else 0, M, x_codes.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
+                          workspace.numel(), _stream()))
+    return y
+
+
+def nvfp4_gemm_pack_act(x_codes, x_scales, xpack=None):
+    """canonical activation codes [M,K/2] / scales [M,K/16] (M <= 128) -> the GEMM's packed records."""
+    M, K = x_codes.shape[0], x_codes.shape[1] * 2
+    if xpack is None:
+        xpack = torch.empty(lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device=x_codes.device)
+    _check(lib.nvfp4_gemm_pack_act(_ptr(x_codes), _ptr(x_scales), M, K, x_codes.stride(0), _ptr(xpack), _stream()))
+    return xpack
+
+
+def nvfp4_quantize_act_packed(x_bf16, xpack=None, gscale=None, gscale_mode=GSCALE_DYNAMIC):
+    """BF16 [M,K] (M <= 128) -> (packed activation records, g f32 [1] or [M])."""
+    M, K = x_bf16.shape
+    if xpack is None:
+        xpack = torch.empty(lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device=x_bf16.device)
+    if gscale is None:
+        gscale = torch.zeros(M if gscale_mode == GSCALE_DYNAMIC_PER_ROW else 1, dtype=torch.float32, device=x_bf16.device)
+    _check(lib.nvfp4_quantize_act_packed(_ptr(x_bf16), M, K, x_bf16.stride(0), _ptr(xpack), _ptr(gscale), gscale_mode,
+                                         _stream()))
+    return xpack, gscale
+
+
+def nvfp4_silu_mul_quantize_packed(gu_bf16, xpack=None, gscale=None, gscale_mode=GSCALE_DYNAMIC, h_out=None):
+    M, I = gu_bf16.shape[0], gu_bf16.shape[1] // 2
+    if xpack is None:
+        xpack = torch.empty(lib.nvfp4_gemm_packed_act_bytes(M, I), dtype=torch.uint8, device=gu_bf16.device)
+    if gscale is None:
+        gscale = torch.zeros(M if gscale_mode == GSCALE_DYNAMIC_PER_ROW else 1, dtype=torch.float32, device=gu_bf16.device)
+    _check(lib.nvfp4_silu_mul_quantize_packed(_ptr(gu_bf16), M, I, _ptr(xpack), _ptr(gscale), gscale_mode, _ptr(h_out),
+                                              _stream()))
+    return xpack, gscale
+
+
+def nvfp4_gemm_packed_new_workspace(M, N, K, device):
+    return torch.zeros(max(16, lib.nvfp4_gemm_packed_workspace_bytes(M, N, K)), dtype=torch.uint8, device=device)
+
+
+def nvfp4_gemm_packed(w_blob_tc, w_gscale, N, K, xpack, x_gscale, M, y=None, y_dtype=DTYPE_BF16, workspace=None,
+                      gscale_per_row=False):
+    """tensor-core W4A4 GEMM on packed activations (M <= 128)."""
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=xpack.device)
+    if workspace is None:
+        workspace = nvfp4_gemm_packed_new_workspace(M, N, K, xpack.device)
+    _check(lib.nvfp4_gemm_packed(_ptr(w_blob_tc), _ptr(w_gscale), N, K, _ptr(xpack), _ptr(x_gscale),
+                                 1 if gscale_per_row else 0, M, _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
+                                 workspace.numel(), _stream()))
     return y
 
 

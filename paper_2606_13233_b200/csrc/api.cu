@@ -271,4 +271,116 @@ int nvfp4_silu_mul(const void* gu_bf16, int M, int I, void* h_bf16, void* stream
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+// ---- tensor-core GEMM (gemm_tc.cu) ----
+size_t nvfp4_gemm_repacked_bytes(int N, int K) {
+    if (N < 1 || K < 1 || !gemm_tc_supported(N, K)) return 0;
+    return gemm_tc_repacked_bytes(N, K);
+}
+
+int nvfp4_gemm_repack_weight(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!codes || !scales || !blob_out) return NVFP4_ERR_INVALID_ARG;
+    if (N < 1 || K < 1 || !gemm_tc_supported(N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(codes) || !aligned16(scales) || !aligned16(blob_out)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_repack_tc(codes, scales, N, K, blob_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemm_unpack_weight(const void* blob, int N, int K, uint8_t* codes_out, uint8_t* scales_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!codes_out || !scales_out || !blob) return NVFP4_ERR_INVALID_ARG;
+    if (N < 1 || K < 1 || !gemm_tc_supported(N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(codes_out) || !aligned16(scales_out) || !aligned16(blob)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_unpack_tc(blob, N, K, codes_out, scales_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+size_t nvfp4_gemm_workspace_bytes(int M, int N, int K) {
+    if (M < 1 || M > (1 << 20) || N < 1 || K < 1 || !gemm_tc_supported(N, K)) return 0;
+    return gemm_tc_workspace_bytes(M, N, K);
+}
+
+int nvfp4_gemm(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* x_codes, const uint8_t* x_scales,
+               const float* x_gscale, int gscale_per_row, int M, int64_t ldx, void* y, int y_dtype, int64_t ldy,
+               void* workspace, size_t ws_bytes, void* stream) {
+    g_last_err[0] = 0;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_per_row != 0 && gscale_per_row != 1) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob_tc || !w_gscale || !x_codes || !x_scales || !x_gscale || !y || !workspace) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > (1 << 20) || N < 1 || K < 1 || !gemm_tc_supported(N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (ldy < N || ldx < K / 2 || (ldx % 16) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob_tc) || !aligned16(x_codes) || !aligned16(x_scales) || !aligned16(y) || !aligned16(workspace) ||
+        (reinterpret_cast<uintptr_t>(w_gscale) & 3u) || (reinterpret_cast<uintptr_t>(x_gscale) & 3u))
+        return NVFP4_ERR_ALIGNMENT;
+    if (ws_bytes < gemm_tc_workspace_bytes(M, N, K)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemm_tc(w_blob_tc, w_gscale, N, K, static_cast<const uint8_t*>(x_codes), ldx, x_scales, x_gscale,
+                                   gscale_per_row, M, y, y_dtype, ldy, workspace, ws_bytes, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+size_t nvfp4_gemm_packed_act_bytes(int M, int K) {
+    if (M < 1 || M > 128 || K < 1 || !gemm_tc_supported(1, K)) return 0;
+    return gemm_tc_packed_act_bytes(M, K);
+}
+
+int nvfp4_gemm_pack_act(const void* x_codes, const uint8_t* x_scales, int M, int K, int64_t ldx, void* xpack_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!x_codes || !x_scales || !xpack_out) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > 128 || K < 1 || !gemm_tc_supported(1, K) || ldx < K / 2 || (ldx % 16) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(x_codes) || !aligned16(x_scales) || !aligned16(xpack_out)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_pack_x(static_cast<const uint8_t*>(x_codes), ldx, x_scales, M, K, xpack_out, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_quantize_act_packed(const void* x_bf16, int M, int K, int64_t ldx, void* xpack_out, float* gscale, int gscale_mode,
+                              void* stream) {
+    g_last_err[0] = 0;
+    if (!x_bf16 || !xpack_out || !gscale) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC &&
+        gscale_mode != NVFP4_GSCALE_DYNAMIC_PER_ROW) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > 128 || K < 1 || !gemm_tc_supported(1, K) || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (gscale_mode == NVFP4_GSCALE_DYNAMIC_PER_ROW && (M > 8 || (int64_t)M * K > 524288)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(x_bf16) || !aligned16(xpack_out) || (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_quantize_act(x_bf16, M, K, ldx, static_cast<uint8_t*>(xpack_out), nullptr, gscale, gscale_mode,
+                                        static_cast<cudaStream_t>(stream), gemm_tc_act_mt(M));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_silu_mul_quantize_packed(const void* gu_bf16, int M, int I, void* xpack_out, float* gscale, int gscale_mode,
+                                   void* h_bf16_opt, void* stream) {
+    g_last_err[0] = 0;
+    if (!gu_bf16 || !xpack_out || !gscale) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC &&
+        gscale_mode != NVFP4_GSCALE_DYNAMIC_PER_ROW) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > 128 || I < 1 || !gemm_tc_supported(1, I) || (int64_t)M * I > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (gscale_mode == NVFP4_GSCALE_DYNAMIC_PER_ROW && M > 8) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(gu_bf16) || !aligned16(xpack_out) || (h_bf16_opt && !aligned16(h_bf16_opt)) ||
+        (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_silu_mul_quantize(gu_bf16, M, I, static_cast<uint8_t*>(xpack_out), nullptr, gscale, gscale_mode,
+                                             h_bf16_opt, static_cast<cudaStream_t>(stream), gemm_tc_act_mt(M));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+size_t nvfp4_gemm_packed_workspace_bytes(int M, int N, int K) {
+    if (M < 1 || M > 128 || N < 1 || K < 1 || !gemm_tc_supported(N, K)) return 0;
+    return gemm_tc_packed_workspace_bytes(M, N, K);
+}
+
+int nvfp4_gemm_packed(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* xpack, const float* x_gscale,
+                      int gscale_per_row, int M, void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes,
+                      void* stream) {
+    g_last_err[0] = 0;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_per_row != 0 && gscale_per_row != 1) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob_tc || !w_gscale || !xpack || !x_gscale || !y || !workspace) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > 128 || N < 1 || K < 1 || !gemm_tc_supported(N, K) || ldy < N) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob_tc) || !aligned16(xpack) || !aligned16(y) || !aligned16(workspace) ||
+        (reinterpret_cast<uintptr_t>(w_gscale) & 3u) || (reinterpret_cast<uintptr_t>(x_gscale) & 3u))
+        return NVFP4_ERR_ALIGNMENT;
+    if (ws_bytes < gemm_tc_packed_workspace_bytes(M, N, K)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemm_tc_packed(w_blob_tc, w_gscale, N, K, xpack, x_gscale, gscale_per_row, M, y, y_dtype, ldy,
+                                          workspace, ws_bytes, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 }  // extern "C"

@@ -47,9 +47,9 @@ inline cudaError_t ensure_dynamic_smem(Kernel kernel, size_t* configured /*[MAX_
 }
 
 cudaError_t launch_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* codes, uint8_t* scales,
-                                float* gscale, int gscale_mode, cudaStream_t st);
+                                float* gscale, int gscale_mode, cudaStream_t st, int pack_mt = 0);
 cudaError_t launch_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, uint8_t* scales, float* gscale,
-                                     int gscale_mode, void* h_bf16_opt, cudaStream_t st);
+                                     int gscale_mode, void* h_bf16_opt, cudaStream_t st, int pack_mt = 0);
 
 cudaError_t launch_repack(const uint8_t* codes, const uint8_t* scales, int N, int K, int kp, void* blob, cudaStream_t st);
 cudaError_t launch_unpack(const void* blob, int N, int K, int kp, uint8_t* codes, uint8_t* scales, cudaStream_t st);
@@ -68,5 +68,23 @@ constexpr int RESET_STATE_BYTES = 160;
 cudaError_t launch_reset_sampler(const void* logits, int logits_bf16, int B, int V, int64_t ld, void* state, float tau0,
                                  float t_low, float t_high, float top_p, int w, int delimiter, unsigned long long seed,
                                  int* token_out, float* diag_out, cudaStream_t st);
+
+// tensor-core GEMM (gemm_tc.cu)
+bool gemm_tc_supported(int N, int K);
+size_t gemm_tc_repacked_bytes(int N, int K);
+size_t gemm_tc_workspace_bytes(int M, int N, int K);
+int gemm_tc_act_mt(int M);
+size_t gemm_tc_packed_act_bytes(int M, int K);
+size_t gemm_tc_packed_workspace_bytes(int M, int N, int K);
+cudaError_t launch_pack_x(const uint8_t* x_codes, int64_t ldx, const uint8_t* x_scales, int M, int K, void* xpack,
+                          cudaStream_t st);
+cudaError_t launch_gemm_tc_packed(const void* blob, const float* w_gscale, int N, int K, const void* xpack,
+                                  const float* x_gscale, int gscale_per_row, int M, void* y, int y_dtype, int64_t ldy,
+                                  void* workspace, size_t ws_bytes, cudaStream_t st);
+cudaError_t launch_repack_tc(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob, cudaStream_t st);
+cudaError_t launch_unpack_tc(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st);
+cudaError_t launch_gemm_tc(const void* blob, const float* w_gscale, int N, int K, const uint8_t* x_codes, int64_t ldx,
+                           const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, void* y, int y_dtype,
+                           int64_t ldy, void* workspace, size_t ws_bytes, cudaStream_t st);
 
 }  // namespace nvfp4

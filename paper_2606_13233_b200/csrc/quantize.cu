@@ -79,11 +79,26 @@ struct LoadSiluMul {
 
 constexpr int QMODE_STATIC = 0, QMODE_DYNAMIC = 1, QMODE_DYNAMIC_PER_ROW = 2;
 
+// where block b = (m, kb) of the result goes.  pack_mt == 0: canonical codes [M,K/2] / scales [M,K/16];
+// pack_mt = MT > 0: the tensor-core GEMM's activation records (gemm_tc.cu: per 256 k a record of MT*128 code bytes in
+// 8-token x 16-byte core matrices + four 512-byte scale chunks in tcgen05.cp order), `codes` = first record.
+__device__ __forceinline__ void store_block(uint8_t* codes, uint8_t* scales, int pack_mt, int b, int m, int kb, uint2 c, uint8_t s) {
+    if (pack_mt == 0) {
+        *reinterpret_cast<uint2*>(codes + (int64_t)b * 8) = c;      // [M,K/2] contiguous: block b -> 8 bytes
+        scales[b] = s;
+    } else {
+        uint8_t* rec = codes + (size_t)(kb >> 4) * (size_t)(pack_mt * 128 + 2048);
+        const int kc = (kb & 15) >> 1;
+        *reinterpret_cast<uint2*>(rec + (size_t)(kc * (pack_mt >> 3) + (m >> 3)) * 128 + (m & 7) * 16 + (kb & 1) * 8) = c;
+        rec[pack_mt * 128 + ((kb & 15) >> 2) * 512 + (m & 31) * 16 + (m >> 5) * 4 + (kb & 3)] = s;
+    }
+}
+
 // One cluster (gridDim.x CTAs == cluster size) covers the whole tensor; BPT blocks per thread.
 template <int BPT, int QMODE, typename Loader>
 __global__ void __launch_bounds__(QTHREADS_MAX)
 quantize_act_kernel(Loader load, int M, int K, uint8_t* __restrict__ codes, uint8_t* __restrict__ scales,
-                    float* __restrict__ gscale) {
+                    float* __restrict__ gscale, int pack_mt) {
     __shared__ uint32_t warp_max[32];
     __shared__ uint32_t row_max[8];                     // per-row mode: CTA-wide row maxima
     __shared__ uint32_t cta_max[QCLUSTER_MAX][8];       // [source CTA][row] (row 0 only in per-tensor mode)
@@ -184,8 +199,8 @@ quantize_act_kernel(Loader load, int M, int K, uint8_t* __restrict__ codes, uint
         if (b < NB) {
             uint2 c; uint8_t s;
             quantize_block(va[i], vb[i], ab[i], g[i], c, s);
-            *reinterpret_cast<uint2*>(codes + (int64_t)b * 8) = c;   // [M,K/2] contiguous: block b -> 8 bytes
-            scales[b] = s;
+            const int kb = b - rowm[i] * kb_per_row;
+            store_block(codes, scales, pack_mt, b, rowm[i], kb, c, s);
         }
     }
 }
@@ -214,7 +229,7 @@ __global__ void __launch_bounds__(1024) amax_kernel(const uint16_t* __restrict__
 
 __global__ void __launch_bounds__(256) quantize_blocks_kernel(const uint16_t* __restrict__ x, int M, int K, int64_t ldx,
                                                               uint8_t* __restrict__ codes, uint8_t* __restrict__ scales,
-                                                              const float* __restrict__ gscale) {
+                                                              const float* __restrict__ gscale, int pack_mt) {
     const int kb_per_row = K >> 4;
     const int NB = M * kb_per_row;
     const float g = *gscale;
@@ -224,14 +239,13 @@ __global__ void __launch_bounds__(256) quantize_blocks_kernel(const uint16_t* __
         const uint4 a = __ldg(p), bb = __ldg(p + 1);
         uint2 c; uint8_t s;
         quantize_block(a, bb, absmax_bits16(a, bb), g, c, s);
-        *reinterpret_cast<uint2*>(codes + (int64_t)b * 8) = c;
-        scales[b] = s;
+        store_block(codes, scales, pack_mt, b, m, kb, c, s);
     }
 }
 
 template <int BPT, int QMODE, typename Loader>
 static cudaError_t launch_cluster(int nctas, int threads, cudaStream_t st, Loader load, int M, int K,
-                                  uint8_t* codes, uint8_t* scales, float* gscale) {
+                                  uint8_t* codes, uint8_t* scales, float* gscale, int pack_mt) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(nctas);
     cfg.blockDim = dim3(threads);
@@ -244,7 +258,7 @@ static cudaError_t launch_cluster(int nctas, int threads, cudaStream_t st, Loade
     attr[0].val.clusterDim.z = 1;
     if (nctas > 1) { cfg.attrs = attr; cfg.numAttrs = 2; }
     else           { cfg.attrs = attr + 1; cfg.numAttrs = 1; }      // single CTA: no cluster launch needed
-    return cudaLaunchKernelEx(&cfg, quantize_act_kernel<BPT, QMODE, Loader>, load, M, K, codes, scales, gscale);
+    return cudaLaunchKernelEx(&cfg, quantize_act_kernel<BPT, QMODE, Loader>, load, M, K, codes, scales, gscale, pack_mt);
 }
 
 // smallest cluster that covers NB blocks with <= 4 blocks per thread; prefer 1 block per thread
@@ -262,8 +276,8 @@ static bool cluster_shape(int NB, int& bpt, int& nctas, int& threads) {
 
 template <typename Loader>
 static cudaError_t launch_cluster_any(int bpt, int qmode, int nctas, int threads, cudaStream_t st, Loader load, int M, int K,
-                                      uint8_t* codes, uint8_t* scales, float* gscale) {
-#define NVFP4_Q_CASE(B, Q) if (bpt == B && qmode == Q) return launch_cluster<B, Q, Loader>(nctas, threads, st, load, M, K, codes, scales, gscale);
+                                      uint8_t* codes, uint8_t* scales, float* gscale, int pack_mt) {
+#define NVFP4_Q_CASE(B, Q) if (bpt == B && qmode == Q) return launch_cluster<B, Q, Loader>(nctas, threads, st, load, M, K, codes, scales, gscale, pack_mt);
     NVFP4_Q_CASE(1, QMODE_STATIC) NVFP4_Q_CASE(1, QMODE_DYNAMIC) NVFP4_Q_CASE(1, QMODE_DYNAMIC_PER_ROW)
     NVFP4_Q_CASE(2, QMODE_STATIC) NVFP4_Q_CASE(2, QMODE_DYNAMIC) NVFP4_Q_CASE(2, QMODE_DYNAMIC_PER_ROW)
     NVFP4_Q_CASE(4, QMODE_STATIC) NVFP4_Q_CASE(4, QMODE_DYNAMIC) NVFP4_Q_CASE(4, QMODE_DYNAMIC_PER_ROW)
@@ -277,7 +291,7 @@ static int qmode_of(int gscale_mode) {
 }
 
 cudaError_t launch_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, uint8_t* codes, uint8_t* scales,
-                                float* gscale, int gscale_mode, cudaStream_t st) {
+                                float* gscale, int gscale_mode, cudaStream_t st, int pack_mt) {
     const uint16_t* x = static_cast<const uint16_t*>(x_bf16);
     const int NB = M * (K / 16);
     const bool dyn = (gscale_mode == NVFP4_GSCALE_DYNAMIC);
@@ -286,20 +300,20 @@ cudaError_t launch_quantize_act(const void* x_bf16, int M, int K, int64_t ldx, u
         if (gscale_mode == NVFP4_GSCALE_DYNAMIC_PER_ROW) return cudaErrorInvalidConfiguration;
         if (dyn) amax_kernel<<<1, 1024, 0, st>>>(x, M, K, ldx, gscale);
         int grid = (NB + 255) / 256; if (grid > 148 * 8) grid = 148 * 8;
-        quantize_blocks_kernel<<<grid, 256, 0, st>>>(x, M, K, ldx, codes, scales, gscale);
+        quantize_blocks_kernel<<<grid, 256, 0, st>>>(x, M, K, ldx, codes, scales, gscale, pack_mt);
         return cudaGetLastError();
     }
-    return launch_cluster_any(bpt, qmode_of(gscale_mode), nctas, threads, st, LoadX{x, ldx}, M, K, codes, scales, gscale);
+    return launch_cluster_any(bpt, qmode_of(gscale_mode), nctas, threads, st, LoadX{x, ldx}, M, K, codes, scales, gscale, pack_mt);
 }
 
 // nvfp4_silu_mul_quantize: h = RN_bf16(silu(gate) * up), then the quantizer on h[M, I] -- one launch
 cudaError_t launch_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, uint8_t* scales, float* gscale,
-                                     int gscale_mode, void* h_bf16_opt, cudaStream_t st) {
+                                     int gscale_mode, void* h_bf16_opt, cudaStream_t st, int pack_mt) {
     const int NB = M * (I / 16);
     int bpt, nctas, threads;
     if (!cluster_shape(NB, bpt, nctas, threads)) return cudaErrorInvalidConfiguration;
     const LoadSiluMul load{static_cast<const uint16_t*>(gu_bf16), I, static_cast<uint16_t*>(h_bf16_opt)};
-    return launch_cluster_any(bpt, qmode_of(gscale_mode), nctas, threads, st, load, M, I, codes, scales, gscale);
+    return launch_cluster_any(bpt, qmode_of(gscale_mode), nctas, threads, st, load, M, I, codes, scales, gscale, pack_mt);
 }
 
 }  // namespace nvfp4
