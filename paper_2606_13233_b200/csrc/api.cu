@@ -318,6 +318,12 @@ int nvfp4_gemm(const void* w_blob_tc, const float* w_gscale, int N, int K, const
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+int nvfp4_gemm_set_config(int stages) {
+    if (stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
+    gemm_tc_set_stages(stages);
+    return NVFP4_OK;
+}
+
 size_t nvfp4_gemm_packed_act_bytes(int M, int K) {
     if (M < 1 || M > 128 || K < 1 || !gemm_tc_supported(1, K)) return 0;
     return gemm_tc_packed_act_bytes(M, K);
