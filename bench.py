@@ -297,6 +297,7 @@ def job_value(bytes_per_rank_step, world, ms_step):
 
 # ---- our arm -----------------------------------------------------------------------------------
 MS = (1, 2, 4, 8)                      # BASELINE.json metric: "at M = 1, 2, 4, 8"
+TC_MS = (1, 2, 4, 8, 16, 32, 64, 128)  # the tensor-core GEMM is timed beside the GEMV up to M = 128
 MIN_REPLAYS = 200                      # timed graph replays, whatever --steps says
 HEAVY_LANES_PER_CLK_SM = 64.0          # IDP.4A / FFMA2 / HFMA2 issue rate (profiles/r02_microbench.md)
 NUM_SMS = 148
@@ -342,6 +343,39 @@ class ShapeBank:
         del g
         return us
 
+    def time_tensor_core(self, Ms, reps_total=MIN_REPLAYS):
+        """cold-L2 us per call of the tcgen05 GEMM (nvfp4_gemm_packed on pre-packed activations) at each M: {M: us}.
+        The tensor-core blobs replace the GEMV blobs of this bank (same canonical bytes, other layout)."""
+        torch, B, N, K = self.torch, self.B, self.N, self.K
+        self.blobs = []
+        torch.cuda.empty_cache()
+        tcb = []
+        for c in range(self.copies):
+            codes, scales, _ = inputs.make_nvfp4_weight_device(N, K, seed=c, shape_id=self.sid)
+            tcb.append(B.nvfp4_gemm_repack_weight(codes, scales))
+            del codes, scales
+        out = {}
+        for M in Ms:
+            xbits = inputs.make_activation_bits(min(M, 8), K, seed=0, shape_id=self.sid)
+            x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
+            x = x.repeat((M + 7) // 8, 1)[:M].contiguous()
+            xp, gx = B.nvfp4_quantize_act_packed(x)
+            y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+            ws = B.nvfp4_gemm_packed_new_workspace(M, N, K, "cuda")
+            call = lambda b: B.nvfp4_gemm_packed(b, self.gw, N, K, xp, gx, M, y=y, y_dtype=B.DTYPE_BF16, workspace=ws)
+            for b in tcb[:2]:
+                call(b)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                for b in tcb:
+                    call(b)
+            out[M] = time_graph(torch, g, max(3, reps_total // self.copies), 3) / self.copies * 1e3
+            del g
+        del tcb
+        torch.cuda.empty_cache()
+        return out
+
     def time_cublas(self, Ms):
         """torch.matmul (cuBLAS) BF16 on BF16 weights of the same shape, same cold rotation: {M: us}."""
         torch, N, K = self.torch, self.N, self.K
@@ -365,17 +399,19 @@ class ShapeBank:
         return out
 
 
-def chain_ms_per_token(M, layers, peak):
+def chain_ms_per_token(M, layers, peak, variants=("two_calls", "fused_quant", "tensor_core")):
     """BASELINE.json configs[4]: `layers` x {QKV, O, gate_up, down} + quantizers + SiLU*mul, distinct weights per layer,
-    one CUDA graph; the best of the chain's launch variants is reported with its name."""
+    one CUDA graph; the best of the chain's launch variants is reported with its name.  Variants: the CUDA-core GEMV
+    with separate quantizers / with the quantizer fused into the GEMV (M = 1), and the tcgen05 GEMM path."""
     import torch
     from paper_2606_13233_b200.chain import DecodeChain
     h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
     res = {}
-    for label, fused in (("two_calls", False), ("fused_quant", True)):
+    for label in variants:
+        fused = label == "fused_quant"
         if fused and M > 1:
             continue
-        ch = DecodeChain(layers=layers, M=M, fused=fused)
+        ch = DecodeChain(layers=layers, M=M, fused=fused, tensor_core=(label == "tensor_core"))
         ch.calibrate(h0)
         ch.step()
         torch.cuda.synchronize()
@@ -492,7 +528,7 @@ def run_ours(args):
     del wl
     torch.cuda.empty_cache()
 
-    per_m, chain, roofline_alu, sampler = {}, None, None, None
+    per_m, chain, roofline_alu, sampler, tensor_core = {}, None, None, None, None
     if rank == 0 and not args.headline_only:
         # ---- the whole metric: the step at M = 1, 2, 4, 8; per shape W4A4 / W4A16 / cuBLAS BF16, cold L2 --------
         for m in MS:
@@ -502,6 +538,7 @@ def run_ours(args):
                 del w2
                 torch.cuda.empty_cache()
         shape_rows = {m: {} for m in MS}
+        tc_rows, tc_cross = {}, {}
         for sid, (name, N, K) in enumerate(SHAPES, start=1):
             bank = ShapeBank(sid, name, N, K)
             cub = bank.time_cublas(MS)
@@ -514,6 +551,14 @@ def run_ours(args):
                     "us": round(us44, 2), "gbs": round(nb44 / us44 / 1e3, 1), "frac": round(nb44 / us44 / 1e3 / peak, 3),
                     "w4a16_us": round(us416, 2), "w4a16_frac": round(nb416 / us416 / 1e3 / peak, 3),
                     "cublas_bf16_us": round(cub[m], 2), "copies": bank.copies}
+            tc = bank.time_tensor_core(TC_MS)
+            for m in TC_MS:
+                nb = N * K * 9 // 16 + m * (K // 2 + K // 16) + m * N * 2
+                tc_rows.setdefault(str(m), {})[name] = {"us": round(tc[m], 2), "frac": round(nb / tc[m] / 1e3 / peak, 3)}
+                if m in shape_rows:
+                    shape_rows[m][name]["tensor_core_us"] = round(tc[m], 2)
+            wins = [m for m in MS if tc[m] < shape_rows[m][name]["us"]]
+            tc_cross[name] = min(wins) if wins else None
             del bank
             torch.cuda.empty_cache()
         for m in MS:
@@ -537,9 +582,21 @@ def run_ours(args):
                                "M = 8; peak = 64 lanes/clk/SM (measured, profiles/r02_microbench.md) x 148 SMs x sampled SM clock",
                         "hbm_frac_same_kernels": per_m["8"]["gemv_only_frac"]}
         sampler = sampler_us_per_token()
+        tensor_core = {
+            "what": "nvfp4_gemm_packed: tcgen05 kind::mxf4nvf4 block-scaled MMA, weights as the A operand (swap-AB), persistent "
+                    "stream-K; same cold-L2 rotation and byte count as per_shape_gemv (SURVEY 8(f) row 3, PAPER.md App. C.3)",
+            "per_m": {m: {"per_shape": rows, "sum_us": round(sum(r["us"] for r in rows.values()), 2)} for m, rows in tc_rows.items()},
+            "gemv_sum_us": {str(m): round(sum(r["us"] for r in shape_rows[m].values()), 2) for m in MS},
+            "crossover_M": tc_cross,
+            "crossover_note": "smallest M in {1,2,4,8} at which the tensor-core kernel is faster than the CUDA-core GEMV on "
+                              "that shape (null: never); the paper's runtime switches at M ~ 16 (PAPER.md:532)",
+            "paper_m128_us": {"qkv": 14.94, "o": 12.74, "gate_up_N25600": 24.99, "down": 24.80,
+                              "ref": "PAPER.md:570-573 Table 16, B200, another machine: context"}}
         if not args.no_chain:
             try:
-                chain = chain_ms_per_token(1, args.layers, peak)
+                chain = chain_ms_per_token(1, args.layers, peak, variants=("two_calls", "fused_quant"))
+                chain["tensor_core_m1"] = chain_ms_per_token(1, args.layers, peak, variants=("tensor_core",))
+                chain["tensor_core_m8"] = chain_ms_per_token(8, args.layers, peak, variants=("tensor_core",))
             except Exception as e:                                        # e.g. not enough free memory on a shared GPU
                 chain = {"unavailable": str(e)[:200]}
 
@@ -567,6 +624,7 @@ def run_ours(args):
             "per_m": per_m,
             "chain": chain,
             "sampler": sampler,
+            "tensor_core": tensor_core,
             "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone)",
                          "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": ach / peak,
                          "traffic": TRAFFIC_BYTES_PER_STEP.get(M),

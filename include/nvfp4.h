@@ -295,7 +295,11 @@ int nvfp4_gemm(const void* w_blob_tc, const float* w_gscale, int N, int K,
  *   nvfp4_silu_mul_quantize_packed  nvfp4_silu_mul_quantize writing the packed layout (M * I <= 524288)
  *   nvfp4_gemm_packed               the GEMM on packed activations; workspace >= nvfp4_gemm_packed_workspace_bytes,
  *                                   zero-filled once; other arguments as for nvfp4_gemm
+ *   nvfp4_gemm_set_config           tuning knobs (0 = table), process-wide like nvfp4_gemv_set_config: depth of the
+ *                                   kernel's shared-memory ring of weight stages (2..16, clamped to what fits) and
+ *                                   the number of persistent CTAs the stage list is cut into (clamped to 148)
  */
+int nvfp4_gemm_set_config(int stages, int ctas);
 size_t nvfp4_gemm_packed_act_bytes(int M, int K);
 int nvfp4_gemm_pack_act(const void* x_codes, const uint8_t* x_scales, int M, int K, int64_t ldx, void* xpack_out, void* stream);
 int nvfp4_quantize_act_packed(const void* x_bf16, int M, int K, int64_t ldx, void* xpack_out, float* gscale, int gscale_mode,

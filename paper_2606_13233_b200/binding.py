@@ -30,7 +30,7 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_gemm_repacked_bytes", "nvfp4_gemm_repack_weight", "nvfp4_gemm_unpack_weight",
            "nvfp4_gemm_workspace_bytes", "nvfp4_gemm", "nvfp4_gemm_packed_act_bytes", "nvfp4_gemm_pack_act",
            "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
-           "nvfp4_gemm_packed")
+           "nvfp4_gemm_packed", "nvfp4_gemm_set_config")
 
 
 class Nvfp4Error(RuntimeError):
@@ -107,6 +107,8 @@ def _load():
     lib.nvfp4_silu_mul_quantize_packed.argtypes = [vp, c_int, c_int, vp, vp, c_int, vp, vp]
     lib.nvfp4_gemm_packed_workspace_bytes.restype = c_sz
     lib.nvfp4_gemm_packed_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemm_set_config.restype = c_int
+    lib.nvfp4_gemm_set_config.argtypes = [c_int, c_int]
     lib.nvfp4_gemm_packed.restype = c_int
     lib.nvfp4_gemm_packed.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, c_int, vp, c_int, c_i64, vp, c_sz, vp]
     return lib
@@ -234,6 +236,10 @@ def nvfp4_gemm(w_blob_tc, w_gscale, N, K, x_codes, x_scales, x_gscale, y=None, y
                           1 if gscale_per_row else 0, M, x_codes.stride(0), _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
                           workspace.numel(), _stream()))
     return y
+
+
+def nvfp4_gemm_set_config(stages=0, ctas=0):
+    _check(lib.nvfp4_gemm_set_config(stages, ctas))
 
 
 def nvfp4_gemm_pack_act(x_codes, x_scales, xpack=None):

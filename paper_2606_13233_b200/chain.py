@@ -20,7 +20,11 @@ QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
 
 class DecodeChain:
     def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False,
-                 fused_producer: bool = True):
+                 fused_producer: bool = True, tensor_core: bool = False):
+        self.tensor_core = tensor_core                # projections on the tcgen05 GEMM (nvfp4_quantize_act_packed +
+                                                      # nvfp4_gemm_packed, M <= 128) instead of the CUDA-core GEMV
+        if tensor_core:
+            fused, fused_producer = False, True
         self.fused = fused                            # one nvfp4_gemv_fused_quant launch per projection
         self.fused_producer = fused_producer          # down's input: nvfp4_silu_mul_quantize (one launch) instead of
                                                       # nvfp4_silu_mul + nvfp4_quantize_act
@@ -36,8 +40,8 @@ class DecodeChain:
                 codes, scales, _ = inputs.make_nvfp4_weight_device(N, K, seed=seed * 1000 + l, shape_id=sid + 1,
                                                                    device=device)
                 g = 1.0 / (557.0 * math.sqrt(K))       # keeps activations O(1) through the chain
-                row.append((B.nvfp4_repack_weight(codes, scales),
-                            torch.tensor([g], dtype=torch.float32, device=device), N, K))
+                blob = B.nvfp4_gemm_repack_weight(codes, scales) if tensor_core else B.nvfp4_repack_weight(codes, scales)
+                row.append((blob, torch.tensor([g], dtype=torch.float32, device=device), N, K))
                 del codes, scales
             self.w.append(row)
         bf, u8 = torch.bfloat16, torch.uint8
@@ -50,7 +54,11 @@ class DecodeChain:
         self.xc = torch.empty((M, kmax // 2), dtype=u8, device=device)   # reused NVFP4 activation buffers
         self.xs = torch.empty((M, kmax // 16), dtype=u8, device=device)
         self.gx = torch.zeros(1, dtype=torch.float32, device=device)
-        self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
+        if tensor_core:
+            self.ws = [B.nvfp4_gemm_packed_new_workspace(M, N, K, device) for _, N, K in self.shapes]
+            self.xpack = torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, kmax), dtype=u8, device=device)
+        else:
+            self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
         self.launches_per_step = layers * ((5 if fused else 8) if fused_producer else (5 if fused else 9))
 
     def set_input(self, h_bf16):
@@ -59,6 +67,10 @@ class DecodeChain:
     def _down_from_gate_up(self, l, y, keep_h=False):
         """down projection fed by the fused producer: SiLU*mul + quantize in one launch, then the W4A4 GEMV."""
         blob, gw, N, K = self.w[l][3]
+        if self.tensor_core:
+            B.nvfp4_silu_mul_quantize_packed(self.y_gu, self.xpack, self.gx, h_out=self.act if keep_h else None)
+            B.nvfp4_gemm_packed(blob, gw, N, K, self.xpack, self.gx, self.M, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[3])
+            return
         xc = self.xc.view(-1)[: self.M * (K // 2)].view(self.M, K // 2)
         xs = self.xs.view(-1)[: self.M * (K // 16)].view(self.M, K // 16)
         B.nvfp4_silu_mul_quantize(self.y_gu, xc, xs, self.gx, h=self.act if keep_h else None)
@@ -66,6 +78,10 @@ class DecodeChain:
 
     def _proj(self, l, i, x, y):
         blob, gw, N, K = self.w[l][i]
+        if self.tensor_core:
+            B.nvfp4_quantize_act_packed(x, self.xpack, self.gx)
+            B.nvfp4_gemm_packed(blob, gw, N, K, self.xpack, self.gx, self.M, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])
+            return
         if self.fused:
             B.nvfp4_gemv_fused_quant(blob, gw, N, K, x, self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])
             return

@@ -318,9 +318,9 @@ int nvfp4_gemm(const void* w_blob_tc, const float* w_gscale, int N, int K, const
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
-int nvfp4_gemm_set_config(int stages) {
-    if (stages < 0 || stages > 16) return NVFP4_ERR_INVALID_ARG;
-    gemm_tc_set_stages(stages);
+int nvfp4_gemm_set_config(int stages, int ctas) {
+    if (stages < 0 || stages > 16 || ctas < 0 || ctas > 1024) return NVFP4_ERR_INVALID_ARG;
+    gemm_tc_set_config(stages, ctas);
     return NVFP4_OK;
 }
 

@@ -70,7 +70,7 @@ cudaError_t launch_reset_sampler(const void* logits, int logits_bf16, int B, int
                                  int* token_out, float* diag_out, cudaStream_t st);
 
 // tensor-core GEMM (gemm_tc.cu)
-void gemm_tc_set_stages(int s);
+void gemm_tc_set_config(int stages, int ctas);
 bool gemm_tc_supported(int N, int K);
 size_t gemm_tc_repacked_bytes(int N, int K);
 size_t gemm_tc_workspace_bytes(int M, int N, int K);

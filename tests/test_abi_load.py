@@ -87,3 +87,30 @@ def test_config_table_is_sane(lib):
     assert lib.nvfp4_set_layout_kparts(0) == 0 and lib.nvfp4_get_layout_kparts(5120, 25600) == 4
     assert lib.nvfp4_get_layout_kparts(51200, 5120) == 1
     assert lib.nvfp4_gemv_set_config(0, 0, 0, 0, 0, 0) == 0
+
+
+def test_gemm_sizes_and_validation_without_gpu(lib):
+    vp, ci, cs = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+    lib.nvfp4_gemm_repacked_bytes.restype = cs
+    lib.nvfp4_gemm_workspace_bytes.restype = cs
+    lib.nvfp4_gemm_packed_act_bytes.restype = cs
+    lib.nvfp4_gemm_packed_workspace_bytes.restype = cs
+    # 128-row tiles x 256-k stages of 18432 B behind the 128-byte header: the canonical information when N % 128 == 0
+    for N, K in [(10240, 5120), (5120, 8192), (51200, 5120), (5120, 25600), (2048, 2048)]:
+        assert lib.nvfp4_gemm_repacked_bytes(N, K) == 128 + N * K // 2 + N * K // 16
+    assert lib.nvfp4_gemm_repacked_bytes(130, 512) == 128 + 2 * 2 * 18432
+    assert lib.nvfp4_gemm_repacked_bytes(128, 384) == 0 and lib.nvfp4_gemm_repacked_bytes(0, 256) == 0
+    # packed activations: per 256 k one record of MT*128 code bytes + 2048 scale bytes, MT = 8, 16, 32, 64, 128 >= M
+    for M, MT in [(1, 8), (8, 8), (9, 16), (17, 32), (33, 64), (65, 128), (128, 128)]:
+        assert lib.nvfp4_gemm_packed_act_bytes(M, 5120) == 20 * (MT * 128 + 2048)
+    assert lib.nvfp4_gemm_packed_act_bytes(129, 5120) == 0 and lib.nvfp4_gemm_packed_act_bytes(1, 100) == 0
+    assert lib.nvfp4_gemm_workspace_bytes(300, 5120, 8192) >= lib.nvfp4_gemm_packed_workspace_bytes(128, 5120, 8192)
+    fake = vp(0x1000)
+    lib.nvfp4_gemm.argtypes = [vp, vp, ci, ci, vp, vp, vp, ci, ci, ctypes.c_int64, vp, ci, ctypes.c_int64, vp, cs, vp]
+    assert lib.nvfp4_gemm(None, fake, 128, 256, fake, fake, fake, 0, 1, 128, fake, 0, 128, fake, 1 << 30, None) == -1
+    assert lib.nvfp4_gemm(fake, fake, 128, 384, fake, fake, fake, 0, 1, 192, fake, 0, 128, fake, 1 << 30, None) == -2
+    assert lib.nvfp4_gemm(fake, fake, 128, 256, fake, fake, fake, 0, 1, 128, fake, 0, 64, fake, 1 << 30, None) == -2   # ldy < N
+    assert lib.nvfp4_gemm(fake, fake, 128, 256, fake, fake, fake, 0, 1, 128, fake, 0, 128, fake, 16, None) == -1       # workspace
+    assert lib.nvfp4_gemm(vp(0x1004), fake, 128, 256, fake, fake, fake, 0, 1, 128, fake, 0, 128, fake, 1 << 30, None) == -3
+    lib.nvfp4_gemm_set_config.argtypes = [ci, ci]
+    assert lib.nvfp4_gemm_set_config(99, 0) == -1 and lib.nvfp4_gemm_set_config(0, 0) == 0

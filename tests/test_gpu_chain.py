@@ -92,3 +92,64 @@ def test_chain_full_size_first_and_last_layer(M):
         ch.step()
     g.replay(); torch.cuda.synchronize()
     assert torch.equal(ch.h, ref)
+
+
+@pytest.mark.parametrize("M", [1, 8, 24])
+def test_chain_tensor_core_small_dims_every_stage(M):
+    """the same chain with every projection on the tcgen05 GEMM (quantize_act_packed / silu_mul_quantize_packed ->
+    gemm_packed): each projection against the oracle on its own downloaded input and unpacked weights."""
+    from paper_2606_13233_b200 import binding as B
+    from paper_2606_13233_b200.chain import DecodeChain
+    dims = dict(hidden=512, qkv=768, o_in=512, inter=768)
+    ch = DecodeChain(layers=2, M=M, dims=dims, seed=6, tensor_core=True)
+    h0 = U.dev_bf16_from_bits(inputs.make_activation_bits(M, 512, 0, 79))
+    ch.calibrate(h0)
+    taps = []
+    ch.step(taps)
+    torch.cuda.synchronize()
+    assert len(taps) == 8
+    for l, name, x, y in taps:
+        i = [s[0] for s in ch.shapes].index(name)
+        blob, gw, N, K = ch.w[l][i]
+        wc, ws = B.nvfp4_gemm_unpack_weight(blob, N, K)
+        xf = orc.bf16_bits_to_f32(U.host_bf16_bits(x.contiguous()))
+        oxc, oxs, ogx = orc.quantize(xf)
+        Y, A = orc.gemv_w4a4(U.host_u8(wc), U.host_u8(ws), np.float32(gw.item()), oxc, oxs, ogx)
+        U.check_gemv(U.host_y_f64(y), Y, A, f"tc chain layer {l} {name} M={M}", bf16_slack=True)
+    ch.set_input(h0); ch.step(); torch.cuda.synchronize()
+    ref = ch.h.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        ch.set_input(h0)
+        ch.step()
+    g.replay(); torch.cuda.synchronize()
+    assert torch.equal(ch.h, ref)
+
+
+def test_chain_tensor_core_full_size_m8():
+    """configs[4] at full size on the tensor-core path, M = 8: first and last layer against the oracle (sampled rows)."""
+    from paper_2606_13233_b200 import binding as B
+    from paper_2606_13233_b200.chain import DecodeChain
+    L, M = 64, 8
+    ch = DecodeChain(layers=L, M=M, seed=11, tensor_core=True)
+    ch.calibrate(U.dev_bf16_from_bits(inputs.make_activation_bits(M, 5120, 0, 80)))
+    taps = []
+    ch.step(taps)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(8)
+    for l, name, x, y in taps:
+        if l not in (0, L - 1):
+            continue
+        i = [s[0] for s in ch.shapes].index(name)
+        blob, gw, N, K = ch.w[l][i]
+        wc, ws = B.nvfp4_gemm_unpack_weight(blob, N, K)
+        rows = np.unique(np.concatenate([np.array([0, 127, 128, N - 1]), rng.integers(0, N, size=60)]))
+        d_rows = torch.from_numpy(rows).cuda()
+        hw, hs = U.host_u8(wc[d_rows]), U.host_u8(ws[d_rows])
+        del wc, ws
+        xf = orc.bf16_bits_to_f32(U.host_bf16_bits(x.contiguous()))
+        assert np.all(np.isfinite(xf)) and np.any(xf != 0)
+        oxc, oxs, ogx = orc.quantize(xf)
+        Y, A = orc.gemv_w4a4(hw, hs, np.float32(gw.item()), oxc, oxs, ogx)
+        U.check_gemv(U.host_y_f64(y)[:, rows], Y, A, f"full-size tc chain layer {l} {name}")
+    assert torch.isfinite(ch.h.float()).all()
