@@ -119,7 +119,7 @@ class Workload:
             blobs = []
             for c in range(copies):
                 codes, scales, g = inputs.make_nvfp4_weight_device(N, K, seed=c, shape_id=sid)
-                blobs.append(B.nvfp4_repack_weight(codes, scales))
+                blobs.append(B.nvfp4_gemm_repack_weight(codes, scales) if mode == "tc" else B.nvfp4_repack_weight(codes, scales))
                 del codes, scales
             xbits = inputs.make_activation_bits(M, K, seed=0, shape_id=sid)
             x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
@@ -131,7 +131,8 @@ class Workload:
                 xs=torch.empty((M, K // 16), dtype=torch.uint8, device="cuda"),
                 gx=torch.zeros(1, dtype=torch.float32, device="cuda"),
                 y=torch.empty((M, N), dtype=torch.bfloat16, device="cuda"),
-                ws=B.new_workspace(M, N, K)))
+                xp=(torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device="cuda") if mode == "tc" else None),
+                ws=(B.nvfp4_gemm_packed_new_workspace(M, N, K, "cuda") if mode == "tc" else B.new_workspace(M, N, K))))
         # e2e staging: the step's four activations / outputs as ONE pinned host buffer and ONE device buffer each
         # (element offsets are multiples of 8 BF16 = 16 B), so a step costs one H2D and one D2H copy
         def pack(key, host_key):
@@ -152,11 +153,17 @@ class Workload:
 
     # -- one projection, all on the current stream ------------------------------------------
     def quantize(self, p):
-        self.B.nvfp4_quantize_act(p["x"], p["xc"], p["xs"], p["gx"])
+        if self.mode == "tc":
+            self.B.nvfp4_quantize_act_packed(p["x"], p["xp"], p["gx"])
+        else:
+            self.B.nvfp4_quantize_act(p["x"], p["xc"], p["xs"], p["gx"])
 
     def gemv(self, p, copy):
         B = self.B
-        if self.mode == "w4a4":
+        if self.mode == "tc":          # the tcgen05 GEMM on packed activations
+            B.nvfp4_gemm_packed(p["blobs"][copy], p["gw"], p["N"], p["K"], p["xp"], p["gx"], self.M, y=p["y"],
+                                y_dtype=B.DTYPE_BF16, workspace=p["ws"])
+        elif self.mode == "w4a4":
             B.nvfp4_gemv(B.MODE_W4A4, p["blobs"][copy], p["gw"], p["N"], p["K"], p["xc"], p["xs"], p["gx"],
                          y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
         else:
@@ -173,7 +180,7 @@ class Workload:
                                               y_dtype=self.B.DTYPE_BF16, workspace=p["ws"])
                 n += 1
                 continue
-            if quant and self.mode == "w4a4":
+            if quant and self.mode in ("w4a4", "tc"):
                 self.quantize(p); n += 1
             if gemv:
                 self.gemv(p, copy); n += 1
@@ -200,7 +207,7 @@ class Workload:
         """public-API path from HOST buffers: H2D activations, quantize, gemv, D2H outputs."""
         self.x_all.copy_(self.x_all_host, non_blocking=True)          # H2D: the step's BF16 activations
         for p in self.proj:
-            if self.mode == "w4a4":
+            if self.mode in ("w4a4", "tc"):
                 self.quantize(p)
             self.gemv(p, copy)
         self.y_all_host.copy_(self.y_all, non_blocking=True)          # D2H: the step's BF16 outputs
@@ -561,6 +568,22 @@ def run_ours(args):
             tc_cross[name] = min(wins) if wins else None
             del bank
             torch.cuda.empty_cache()
+        tc_step = {}
+        for m in MS:
+            w2 = Workload(m, copies=2, mode="tc")
+            g_s, _ = w2.capture(2)
+            g_g, _ = w2.capture(2, quant=False)
+            tc_step[m] = (time_graph(torch, g_s, reps, wrep) / 2, time_graph(torch, g_g, reps, wrep) / 2)
+            if m == M:      # end to end from pinned host buffers on the tensor-core path, as for the headline
+                g_e = torch.cuda.CUDAGraph()
+                w2.step_e2e(0); w2.step_e2e(1); torch.cuda.synchronize()
+                with torch.cuda.graph(g_e):
+                    w2.step_e2e(0)
+                    w2.step_e2e(1)
+                tc_e2e_ms = time_graph(torch, g_e, reps, wrep) / 2
+                del g_e
+            del w2, g_s, g_g
+            torch.cuda.empty_cache()
         for m in MS:
             t_step, t_gemv, t_q, t_fused = step_by_m[m]
             bs = sum(algorithmic_bytes(m, N, K, True) for _, N, K in SHAPES)
@@ -568,6 +591,8 @@ def run_ours(args):
             per_m[str(m)] = {"ms_per_step": round(t_step, 5), "value": round(bs / (t_step * 1e-3) / 1e9, 1), "unit": UNIT,
                              "gemv_only_ms": round(t_gemv, 5), "gemv_only_frac": round(bg / (t_gemv * 1e-3) / 1e9 / peak, 3),
                              "quantize_only_ms": round(t_q, 5), "fused_step_ms": round(t_fused, 5),
+                             "tensor_core_step_ms": round(tc_step[m][0], 5), "tensor_core_gemm_only_ms": round(tc_step[m][1], 5),
+                             "tensor_core_gemm_only_frac": round(bg / (tc_step[m][1] * 1e-3) / 1e9 / peak, 3),
                              "per_shape_gemv": shape_rows[m]}
         # ---- ALU roofline of the integer path at M = 8 (derivation in DESIGN.md section 7) ----------
         clk_mhz = clk.summary()["sm_mhz"] or 1965.0
@@ -587,6 +612,7 @@ def run_ours(args):
                     "stream-K; same cold-L2 rotation and byte count as per_shape_gemv (SURVEY 8(f) row 3, PAPER.md App. C.3)",
             "per_m": {m: {"per_shape": rows, "sum_us": round(sum(r["us"] for r in rows.values()), 2)} for m, rows in tc_rows.items()},
             "gemv_sum_us": {str(m): round(sum(r["us"] for r in shape_rows[m].values()), 2) for m in MS},
+            "e2e_ms_per_step": round(tc_e2e_ms, 5), "e2e_value": round(b_step / (tc_e2e_ms * 1e-3) / 1e9, 1),
             "crossover_M": tc_cross,
             "crossover_note": "smallest M in {1,2,4,8} at which the tensor-core kernel is faster than the CUDA-core GEMV on "
                               "that shape (null: never); the paper's runtime switches at M ~ 16 (PAPER.md:532)",
@@ -646,9 +672,9 @@ def run_ours(args):
 
 # per-step DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum of the 4 GEMV launches) from the committed
 # `ncu --set full` capture of the same kernels; a constant taken from that file, NOT produced by this run.
-TRAFFIC_BYTES_PER_STEP = {1: 280.11e6}
-TRAFFIC_SOURCE = ("constant from profiles/r02_ncu_full_m1.md (ncu --set full capture of the 4 GEMV launches of this step; "
-                  "algorithmic: 274.4 MB); not measured by this run")
+TRAFFIC_BYTES_PER_STEP = {1: 279.68e6}
+TRAFFIC_SOURCE = ("constant from profiles/r02_ncu_full.md (ncu --set full capture of the 4 GEMV launches of this step; "
+                  "algorithmic: 274.4 MB; the tensor-core path: 280.09 MB); not measured by this run")
 
 
 def sweep(wl0, peak):
@@ -761,7 +787,7 @@ def main():
     ap.add_argument("--headline-only", action="store_true", help="only the configs[1] step at --m rows (no per_m table)")
     ap.add_argument("--profile-shape", default=None, help="qkv|o|gate_up|down|all: plain stream launches of "
                     "quantize_act + gemv on that shape only (for ncu); prints a short JSON line")
-    ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16"])
+    ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16", "tc"], help="profile leg: CUDA-core W4A4 / W4A16 GEMV, or tc = the tcgen05 GEMM path")
     ap.add_argument("--chain", action="store_true", help="configs[4]: decode-step projection chain, M = 1,2,4,8")
     ap.add_argument("--layers", type=int, default=64)
     args = ap.parse_args()
