@@ -311,6 +311,25 @@ int nvfp4_gemm_packed(const void* w_blob_tc, const float* w_gscale, int N, int K
                       int gscale_per_row, int M, void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes,
                       void* stream);
 
+/*
+ * nvfp4_gemv for callers that cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments and results as nvfp4_gemv, but the scratch (arrival counters + split partials)
+ * is a built-in array of NVFP4_NOALLOC_SCRATCH_BYTES bytes of device memory that every GPU loading the library holds
+ * until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree): it clears the bytes it is going to
+ * use on `stream`, then launches the same kernel as nvfp4_gemv on that array.
+ *   - shapes whose workspace (nvfp4_gemv_workspace_bytes(M, N, K)) exceeds NVFP4_NOALLOC_SCRATCH_BYTES return
+ *     NVFP4_ERR_UNSUPPORTED_SHAPE (text in nvfp4_last_cuda_error()); 4 MiB covers every Qwen3-8B/14B/32B projection at
+ *     M <= 8 (largest: gate_up 51200 x 5120, M = 8: 3.3 MB), not a 151936-row output head at M = 8
+ *   - EVERY call on a device shares the one array: calls that overlap on the GPU (different streams) race; issue them
+ *     on one stream or order them with events
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress, which may load the
+ *     module): make it outside stream capture
+ */
+#define NVFP4_NOALLOC_SCRATCH_BYTES (4u << 20)
+int nvfp4_gemv_noalloc(int mode, const void* w_blob, const float* w_gscale, int N, int K,
+                       const void* x, const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx,
+                       void* y, int y_dtype, int64_t ldy, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,7 +30,7 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_gemm_repacked_bytes", "nvfp4_gemm_repack_weight", "nvfp4_gemm_unpack_weight",
            "nvfp4_gemm_workspace_bytes", "nvfp4_gemm", "nvfp4_gemm_packed_act_bytes", "nvfp4_gemm_pack_act",
            "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
-           "nvfp4_gemm_packed", "nvfp4_gemm_set_config")
+           "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc")
 
 
 class Nvfp4Error(RuntimeError):
@@ -107,6 +107,8 @@ def _load():
     lib.nvfp4_silu_mul_quantize_packed.argtypes = [vp, c_int, c_int, vp, vp, c_int, vp, vp]
     lib.nvfp4_gemm_packed_workspace_bytes.restype = c_sz
     lib.nvfp4_gemm_packed_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemv_noalloc.restype = c_int
+    lib.nvfp4_gemv_noalloc.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp]
     lib.nvfp4_gemm_set_config.restype = c_int
     lib.nvfp4_gemm_set_config.argtypes = [c_int, c_int]
     lib.nvfp4_gemm_packed.restype = c_int
@@ -288,6 +290,20 @@ def nvfp4_gemm_packed(w_blob_tc, w_gscale, N, K, xpack, x_gscale, M, y=None, y_d
     _check(lib.nvfp4_gemm_packed(_ptr(w_blob_tc), _ptr(w_gscale), N, K, _ptr(xpack), _ptr(x_gscale),
                                  1 if gscale_per_row else 0, M, _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
                                  workspace.numel(), _stream()))
+    return y
+
+
+NOALLOC_SCRATCH_BYTES = 4 << 20
+
+
+def nvfp4_gemv_noalloc(mode, w_blob, w_gscale, N, K, x, x_scales=None, x_gscale=None, y=None, y_dtype=DTYPE_BF16):
+    """nvfp4_gemv on the library's built-in scratch array (no workspace argument, nothing allocated by the call; `y` is
+    the caller's, pass it in when the caller must not allocate either)."""
+    M = x.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x.device)
+    _check(lib.nvfp4_gemv_noalloc(mode, _ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x), _ptr(x_scales), _ptr(x_gscale), M,
+                                  x.stride(0), _ptr(y), y_dtype, y.stride(0), _stream()))
     return y
 
 

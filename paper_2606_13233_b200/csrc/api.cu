@@ -29,6 +29,11 @@ static int effective_kparts(int N, int K) {
     return kp > 0 ? kp : layout_kparts(N, K);
 }
 
+namespace nvfp4 {
+// lets the other translation units of the library (noalloc.cu) leave a message for nvfp4_last_cuda_error()
+void set_last_error(const char* msg) { snprintf(g_last_err, sizeof(g_last_err), "%s", msg); }
+}  // namespace nvfp4
+
 static int cuda_fail(cudaError_t e) {
     snprintf(g_last_err, sizeof(g_last_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
     (void)cudaGetLastError();                     // clear the sticky-less error state

@@ -69,6 +69,8 @@ cudaError_t launch_reset_sampler(const void* logits, int logits_bf16, int B, int
                                  float t_low, float t_high, float top_p, int w, int delimiter, unsigned long long seed,
                                  int* token_out, float* diag_out, cudaStream_t st);
 
+void set_last_error(const char* msg);          // api.cu: text returned by nvfp4_last_cuda_error() (thread-local)
+
 // tensor-core GEMM (gemm_tc.cu)
 void gemm_tc_set_config(int stages, int ctas);
 bool gemm_tc_supported(int N, int K);
