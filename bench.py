@@ -752,9 +752,11 @@ def run_chain(args):
     import torch
     from paper_2606_13233_b200.chain import DecodeChain
     peak, _ = measured_peak()
-    for M, fused, producer in ((1, False, True), (2, False, True), (4, False, True), (8, False, True), (1, True, True),
-                               (1, False, False), (1, True, False)):
-        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer)
+    for M, fused, producer, tc in ((1, False, True, False), (2, False, True, False), (4, False, True, False), (8, False, True, False),
+                                   (1, True, True, False), (1, False, False, False), (1, True, False, False),
+                                   (1, False, True, True), (2, False, True, True), (4, False, True, True), (8, False, True, True),
+                                   (32, False, True, True)):
+        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer, tensor_core=tc)
         h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
         ch.calibrate(h0)
         ch.step()
@@ -766,7 +768,7 @@ def run_chain(args):
         ms = time_graph(torch, g, 20, 3)
         finite = bool(torch.isfinite(ch.h.float()).all())
         wb = ch.weight_bytes()
-        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "fused_quant": fused, "fused_producer": producer, "ms_per_token": round(ms, 4),
+        print(json.dumps({"chain": "qwen3-32b projections", "layers": args.layers, "M": M, "fused_quant": fused, "fused_producer": producer, "tensor_core": tc, "ms_per_token": round(ms, 4),
                           "us_per_layer": round(ms * 1e3 / args.layers, 2), "weight_gb": round(wb / 1e9, 2),
                           "gbs": round(wb / ms / 1e6, 1), "frac_of_copy_peak": round(wb / ms / 1e6 / peak, 3),
                           "launches": ch.launches_per_step, "finite": finite}), flush=True)

@@ -68,7 +68,11 @@ class DecodeChain:
         """down projection fed by the fused producer: SiLU*mul + quantize in one launch, then the W4A4 GEMV."""
         blob, gw, N, K = self.w[l][3]
         if self.tensor_core:
-            B.nvfp4_silu_mul_quantize_packed(self.y_gu, self.xpack, self.gx, h_out=self.act if keep_h else None)
+            if self.M * K <= 524288:                      # the one-launch producer holds the whole [M, I] tensor in one cluster
+                B.nvfp4_silu_mul_quantize_packed(self.y_gu, self.xpack, self.gx, h_out=self.act if keep_h else None)
+            else:
+                B.nvfp4_silu_mul(self.y_gu, self.act)
+                B.nvfp4_quantize_act_packed(self.act, self.xpack, self.gx)
             B.nvfp4_gemm_packed(blob, gw, N, K, self.xpack, self.gx, self.M, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[3])
             return
         xc = self.xc.view(-1)[: self.M * (K // 2)].view(self.M, K // 2)
