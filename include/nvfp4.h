@@ -330,6 +330,23 @@ int nvfp4_gemv_noalloc(int mode, const void* w_blob, const float* w_gscale, int 
                        const void* x, const uint8_t* x_scales, const float* x_gscale, int M, int64_t ldx,
                        void* y, int y_dtype, int64_t ldy, void* stream);
 
+/*
+ * nvfp4_gemm_packed with the NEXT projection's activation quantizer fused into its epilogue (SURVEY.md 8(f) item 1:
+ * "quantize fused into the previous kernel's epilogue when the output tile holds whole 16-blocks and a static global
+ * scale is used"; the paper's deployed flow uses static, calibrated activation scales).  The first
+ * n_quant output columns (n_quant % 256 == 0, <= N) are rounded to BF16 and quantised with the STATIC global scale
+ * *out_gscale (device float, read) by the same binary32 sequence as nvfp4_quantize_act, and written as packed
+ * activation records for a following nvfp4_gemm_packed with K = n_quant and the same M:
+ *   xpack_out == nvfp4_gemm_pack_act(nvfp4_quantize_act(STATIC, RN_bf16(y)[:, :n_quant]))  byte for byte (tokens < M).
+ * xpack_out: nvfp4_gemm_packed_act_bytes(M, n_quant) bytes, 16-byte aligned.  y_opt may be NULL (no BF16 / FP32 output is
+ * written then: the quantised records are the only result).  Values beyond the static scale's range saturate
+ * (block scale clamps at 448, codes at +-6), as in nvfp4_quantize_act(STATIC).  Other arguments as for nvfp4_gemm_packed.
+ */
+int nvfp4_gemm_packed_quant_out(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* xpack,
+                                const float* x_gscale, int gscale_per_row, int M, void* y_opt, int y_dtype, int64_t ldy,
+                                void* xpack_out, const float* out_gscale, int n_quant, void* workspace, size_t ws_bytes,
+                                void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,7 +30,7 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_gemm_repacked_bytes", "nvfp4_gemm_repack_weight", "nvfp4_gemm_unpack_weight",
            "nvfp4_gemm_workspace_bytes", "nvfp4_gemm", "nvfp4_gemm_packed_act_bytes", "nvfp4_gemm_pack_act",
            "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
-           "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc")
+           "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc", "nvfp4_gemm_packed_quant_out")
 
 
 class Nvfp4Error(RuntimeError):
@@ -107,6 +107,9 @@ def _load():
     lib.nvfp4_silu_mul_quantize_packed.argtypes = [vp, c_int, c_int, vp, vp, c_int, vp, vp]
     lib.nvfp4_gemm_packed_workspace_bytes.restype = c_sz
     lib.nvfp4_gemm_packed_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemm_packed_quant_out.restype = c_int
+    lib.nvfp4_gemm_packed_quant_out.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, c_int,
+                                                vp, c_sz, vp]
     lib.nvfp4_gemv_noalloc.restype = c_int
     lib.nvfp4_gemv_noalloc.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp]
     lib.nvfp4_gemm_set_config.restype = c_int
@@ -291,6 +294,23 @@ def nvfp4_gemm_packed(w_blob_tc, w_gscale, N, K, xpack, x_gscale, M, y=None, y_d
                                  1 if gscale_per_row else 0, M, _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
                                  workspace.numel(), _stream()))
     return y
+
+
+def nvfp4_gemm_packed_quant_out(w_blob_tc, w_gscale, N, K, xpack, x_gscale, M, out_gscale, n_quant=None, xpack_out=None, y=None,
+                                y_dtype=DTYPE_BF16, workspace=None, gscale_per_row=False):
+    """nvfp4_gemm_packed whose epilogue also quantises the first n_quant output columns with the STATIC global scale
+    out_gscale into packed records for the next GEMM.  `y` optional (None: only the records are written).
+    Returns (xpack_out, y)."""
+    n_quant = N if n_quant is None else n_quant
+    if xpack_out is None:
+        xpack_out = torch.empty(lib.nvfp4_gemm_packed_act_bytes(M, n_quant), dtype=torch.uint8, device=xpack.device)
+    if workspace is None:
+        workspace = nvfp4_gemm_packed_new_workspace(M, N, K, xpack.device)
+    _check(lib.nvfp4_gemm_packed_quant_out(_ptr(w_blob_tc), _ptr(w_gscale), N, K, _ptr(xpack), _ptr(x_gscale),
+                                           1 if gscale_per_row else 0, M, _ptr(y), y_dtype, y.stride(0) if y is not None else N,
+                                           _ptr(xpack_out), _ptr(out_gscale), n_quant, _ptr(workspace), workspace.numel(),
+                                           _stream()))
+    return xpack_out, y
 
 
 NOALLOC_SCRATCH_BYTES = 4 << 20

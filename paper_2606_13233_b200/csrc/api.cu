@@ -394,4 +394,23 @@ int nvfp4_gemm_packed(const void* w_blob_tc, const float* w_gscale, int N, int K
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+int nvfp4_gemm_packed_quant_out(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* xpack,
+                                const float* x_gscale, int gscale_per_row, int M, void* y_opt, int y_dtype, int64_t ldy,
+                                void* xpack_out, const float* out_gscale, int n_quant, void* workspace, size_t ws_bytes,
+                                void* stream) {
+    g_last_err[0] = 0;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_per_row != 0 && gscale_per_row != 1) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob_tc || !w_gscale || !xpack || !x_gscale || !xpack_out || !out_gscale || !workspace) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > 128 || N < 1 || K < 1 || !gemm_tc_supported(N, K) || (y_opt && ldy < N)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (n_quant < 256 || n_quant > N || (n_quant % 256) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob_tc) || !aligned16(xpack) || (y_opt && !aligned16(y_opt)) || !aligned16(xpack_out) || !aligned16(workspace) ||
+        (reinterpret_cast<uintptr_t>(w_gscale) & 3u) || (reinterpret_cast<uintptr_t>(x_gscale) & 3u) ||
+        (reinterpret_cast<uintptr_t>(out_gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    if (ws_bytes < gemm_tc_packed_workspace_bytes(M, N, K)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemm_tc_packed(w_blob_tc, w_gscale, N, K, xpack, x_gscale, gscale_per_row, M, y_opt, y_dtype, ldy,
+                                          workspace, ws_bytes, static_cast<cudaStream_t>(stream), xpack_out, out_gscale, n_quant);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 }  // extern "C"

@@ -192,3 +192,60 @@ def test_silu_mul_quantize_packed(B):
     buf = torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(M, I), dtype=torch.uint8, device="cuda")
     got, g2 = B.nvfp4_silu_mul_quantize_packed(gu, xpack=buf)
     assert np.array_equal(U.host_u8(got), want) and torch.equal(g, g2)
+
+
+@pytest.mark.parametrize("M,N,K,nq", [(1, 512, 512, 512), (8, 1024, 2048, 768), (5, 5120, 1024, 5120), (24, 768, 512, 256),
+                                       (100, 512, 768, 512), (4, 10240, 5120, 8192), (8, 5120, 8192, 5120)])
+def test_fused_output_quantizer_equals_separate_quantizer_and_oracle(B, M, N, K, nq):
+    """nvfp4_gemm_packed_quant_out: the packed records its epilogue writes == pack_act(quantize_act(STATIC) of the BF16
+    output of the plain GEMM) byte for byte, and == the oracle's STATIC quantisation of that output; the optional y equals
+    the plain GEMM's.  Covers whole tiles, K-sliced tiles (fix-up paths) and the bulk fix-up (M > 8)."""
+    c = make_case(M, N, K, seed=N + K + M)
+    blob = B.nvfp4_gemm_repack_weight(U.dev_u8(c["wc"]), U.dev_u8(c["ws"]))
+    xp = B.nvfp4_gemm_pack_act(U.dev_u8(c["xc"]), U.dev_u8(c["xs"]))
+    gw, gx = U.dev_f32(c["gw"]), U.dev_f32(c["gx"])
+    y_ref = B.nvfp4_gemm_packed(blob, gw, N, K, xp, gx, M, y_dtype=B.DTYPE_BF16)
+    torch.cuda.synchronize()
+    yf = orc.bf16_bits_to_f32(U.host_bf16_bits(y_ref))[:, :nq]
+    # a static scale as a calibration would give it: from the tensor's amax, made a bit too small so that some blocks saturate
+    g_static = np.float32(np.max(np.abs(yf)) / 2688.0 * 0.8)
+    d_g = U.dev_f32(g_static)
+    out = torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(M, nq), dtype=torch.uint8, device="cuda")
+    y = torch.zeros((M, N), dtype=torch.bfloat16, device="cuda")
+    B.nvfp4_gemm_packed_quant_out(blob, gw, N, K, xp, gx, M, d_g, n_quant=nq, xpack_out=out, y=y)
+    torch.cuda.synchronize()
+    assert torch.equal(y, y_ref)
+    # the separate GPU quantizer (STATIC, packed output) on the same BF16 values
+    want = torch.zeros_like(out)
+    B.nvfp4_quantize_act_packed(y_ref[:, :nq].contiguous(), xpack=want, gscale=d_g.clone(), gscale_mode=B.GSCALE_STATIC)
+    torch.cuda.synchronize()
+    assert torch.equal(out, want)
+    # and the oracle's STATIC quantisation of those values, packed
+    oc, os_, _ = orc.quantize(yf, g=g_static)
+    assert torch.equal(out, B.nvfp4_gemm_pack_act(U.dev_u8(oc), U.dev_u8(os_)))
+    assert np.any(os_ == 0x7E) or M * nq < 4096          # the 0.8 factor does make some block scales clamp
+    # records only, no y
+    out2 = torch.zeros_like(out)
+    B.nvfp4_gemm_packed_quant_out(blob, gw, N, K, xp, gx, M, d_g, n_quant=nq, xpack_out=out2, y=None)
+    torch.cuda.synchronize()
+    assert torch.equal(out2, want)
+
+
+def test_fused_output_quantizer_feeds_next_gemm(B):
+    """two projections back to back with no quantizer launch in between: GEMM1 (+ fused quantizer) -> GEMM2, against the
+    oracle run on GEMM1's BF16 output."""
+    M, K1, N1, N2 = 6, 1024, 1536, 640
+    c = make_case(M, N1, K1, seed=31)
+    w2c, w2s, g2 = U.oracle_weight(N2, N1, 32, 0)
+    blob1 = B.nvfp4_gemm_repack_weight(U.dev_u8(c["wc"]), U.dev_u8(c["ws"]))
+    blob2 = B.nvfp4_gemm_repack_weight(U.dev_u8(w2c), U.dev_u8(w2s))
+    xp = B.nvfp4_gemm_pack_act(U.dev_u8(c["xc"]), U.dev_u8(c["xs"]))
+    y1 = torch.zeros((M, N1), dtype=torch.bfloat16, device="cuda")
+    g_mid = U.dev_f32(np.float32(0.004))
+    mid, _ = B.nvfp4_gemm_packed_quant_out(blob1, U.dev_f32(c["gw"]), N1, K1, xp, U.dev_f32(c["gx"]), M, g_mid, y=y1)
+    y2 = B.nvfp4_gemm_packed(blob2, U.dev_f32(g2), N2, N1, mid, g_mid, M, y_dtype=B.DTYPE_F32)
+    torch.cuda.synchronize()
+    y1f = orc.bf16_bits_to_f32(U.host_bf16_bits(y1))
+    oc, os_, og = orc.quantize(y1f, g=np.float32(0.004))
+    Y2, A2 = orc.gemv_w4a4(w2c, w2s, g2, oc, os_, og)
+    U.check_gemv(U.host_y_f64(y2), Y2, A2, "GEMM2 on records written by GEMM1's epilogue")
