@@ -418,7 +418,8 @@ def chain_ms_per_token(M, layers, peak, variants=("two_calls", "fused_quant", "t
         fused = label == "fused_quant"
         if fused and M > 1:
             continue
-        ch = DecodeChain(layers=layers, M=M, fused=fused, tensor_core=(label == "tensor_core"))
+        ch = DecodeChain(layers=layers, M=M, fused=fused, tensor_core=label.startswith("tensor_core"),
+                         static_scales=(label == "tensor_core_static"))
         ch.calibrate(h0)
         ch.step()
         torch.cuda.synchronize()
@@ -621,8 +622,8 @@ def run_ours(args):
         if not args.no_chain:
             try:
                 chain = chain_ms_per_token(1, args.layers, peak, variants=("two_calls", "fused_quant"))
-                chain["tensor_core_m1"] = chain_ms_per_token(1, args.layers, peak, variants=("tensor_core",))
-                chain["tensor_core_m8"] = chain_ms_per_token(8, args.layers, peak, variants=("tensor_core",))
+                chain["tensor_core_m1"] = chain_ms_per_token(1, args.layers, peak, variants=("tensor_core", "tensor_core_static"))
+                chain["tensor_core_m8"] = chain_ms_per_token(8, args.layers, peak, variants=("tensor_core", "tensor_core_static"))
             except Exception as e:                                        # e.g. not enough free memory on a shared GPU
                 chain = {"unavailable": str(e)[:200]}
 
@@ -752,11 +753,12 @@ def run_chain(args):
     import torch
     from paper_2606_13233_b200.chain import DecodeChain
     peak, _ = measured_peak()
-    for M, fused, producer, tc in ((1, False, True, False), (2, False, True, False), (4, False, True, False), (8, False, True, False),
-                                   (1, True, True, False), (1, False, False, False), (1, True, False, False),
-                                   (1, False, True, True), (2, False, True, True), (4, False, True, True), (8, False, True, True),
-                                   (32, False, True, True)):
-        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer, tensor_core=tc)
+    for M, fused, producer, tc in ((1, False, True, 0), (2, False, True, 0), (4, False, True, 0), (8, False, True, 0),
+                                   (1, True, True, 0), (1, False, False, 0), (1, True, False, 0),
+                                   (1, False, True, 1), (2, False, True, 1), (4, False, True, 1), (8, False, True, 1), (32, False, True, 1),
+                                   (1, False, True, 2), (2, False, True, 2), (4, False, True, 2), (8, False, True, 2), (32, False, True, 2)):
+        # tc: 0 = CUDA-core GEMV, 1 = tensor-core GEMM with quantizer launches, 2 = tensor-core GEMM, static scales, fused quantizers
+        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer, tensor_core=tc > 0, static_scales=tc == 2)
         h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
         ch.calibrate(h0)
         ch.step()

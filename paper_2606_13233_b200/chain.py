@@ -20,7 +20,11 @@ QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
 
 class DecodeChain:
     def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False,
-                 fused_producer: bool = True, tensor_core: bool = False):
+                 fused_producer: bool = True, tensor_core: bool = False, static_scales: bool = False):
+        # static_scales (tensor-core path only; the paper's deployed flow): every projection's input global
+        # scale is fixed by calibrate(), and each GEMM quantises the NEXT projection's input in its own epilogue
+        # (nvfp4_gemm_packed_quant_out): 5 launches per layer -- 4 GEMMs + the SiLU*mul/quantize producer
+        self.static_scales = static_scales and tensor_core
         self.tensor_core = tensor_core                # projections on the tcgen05 GEMM (nvfp4_quantize_act_packed +
                                                       # nvfp4_gemm_packed, M <= 128) instead of the CUDA-core GEMV
         if tensor_core:
@@ -57,9 +61,13 @@ class DecodeChain:
         if tensor_core:
             self.ws = [B.nvfp4_gemm_packed_new_workspace(M, N, K, device) for _, N, K in self.shapes]
             self.xpack = torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, kmax), dtype=u8, device=device)
+            self.xpack2 = torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, kmax), dtype=u8, device=device)
+            self.gs = [[torch.zeros(1, dtype=torch.float32, device=device) for _ in self.shapes] for _ in range(layers)]
         else:
             self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
         self.launches_per_step = layers * ((5 if fused else 8) if fused_producer else (5 if fused else 9))
+        if self.static_scales:
+            self.launches_per_step = 1 + (5 if M * I <= 524288 else 6) * layers
 
     def set_input(self, h_bf16):
         self.h.copy_(h_bf16)
@@ -94,9 +102,43 @@ class DecodeChain:
         B.nvfp4_quantize_act(x, xc, xs, self.gx)
         B.nvfp4_gemv(B.MODE_W4A4, blob, gw, N, K, xc, xs, self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])
 
+    def _step_static(self, taps=None):
+        """tensor-core chain with static activation scales: one quantizer launch for the token's input, then per layer
+        QKV(+quant for O) -> O(+quant for gate_up) -> gate_up -> SiLU*mul+quantize -> down(+quant for the next QKV)."""
+        d, M, S = self.d, self.M, B.GSCALE_STATIC
+        H, OIN, I = d["hidden"], d["o_in"], d["inter"]
+        keep = taps is not None
+        a, b = self.xpack, self.xpack2
+        B.nvfp4_quantize_act_packed(self.h, a, self.gs[0][0], gscale_mode=S)
+        for l in range(self.layers):
+            (bq, gq, Nq, Kq), (bo, go, No, Ko), (bg, gg, Ng, Kg), (bd, gd, Nd, Kd) = self.w[l]
+            x_in = self.h.clone() if keep else None
+            B.nvfp4_gemm_packed_quant_out(bq, gq, Nq, Kq, a, self.gs[l][0], M, self.gs[l][1], n_quant=OIN, xpack_out=b,
+                                          y=self.y_qkv if keep else None, workspace=self.ws[0])
+            B.nvfp4_gemm_packed_quant_out(bo, go, No, Ko, b, self.gs[l][1], M, self.gs[l][2], n_quant=H, xpack_out=a,
+                                          y=self.y_o if keep else None, workspace=self.ws[1])
+            B.nvfp4_gemm_packed(bg, gg, Ng, Kg, a, self.gs[l][2], M, y=self.y_gu, y_dtype=B.DTYPE_BF16, workspace=self.ws[2])
+            if M * I <= 524288:
+                B.nvfp4_silu_mul_quantize_packed(self.y_gu, b, self.gs[l][3], gscale_mode=S, h_out=self.act if keep else None)
+            else:
+                B.nvfp4_silu_mul(self.y_gu, self.act)
+                B.nvfp4_quantize_act_packed(self.act, b, self.gs[l][3], gscale_mode=S)
+            if l + 1 < self.layers:
+                B.nvfp4_gemm_packed_quant_out(bd, gd, Nd, Kd, b, self.gs[l][3], M, self.gs[l + 1][0], n_quant=H, xpack_out=a,
+                                              y=self.h if keep else None, workspace=self.ws[3])
+            else:
+                B.nvfp4_gemm_packed(bd, gd, Nd, Kd, b, self.gs[l][3], M, y=self.h, y_dtype=B.DTYPE_BF16, workspace=self.ws[3])
+            if keep:
+                taps.append((l, "qkv", x_in, self.y_qkv.clone()))
+                taps.append((l, "o", self.y_qkv[:, :OIN].clone(), self.y_o.clone()))
+                taps.append((l, "gate_up", self.y_o.clone(), self.y_gu.clone()))
+                taps.append((l, "down", self.act.clone(), self.h.clone()))
+
     def step(self, taps=None):
         """enqueue the whole chain once; `taps` (tests) collects (layer, name, input clone, output clone)."""
         d = self.d
+        if self.static_scales:
+            return self._step_static(taps)
         for l in range(self.layers):
             stages = (("qkv", self.h, self.y_qkv), ("o", self.y_qkv[:, : d["o_in"]], self.y_o),
                       ("gate_up", self.y_o, self.y_gu), ("down", self.act, self.h))
@@ -129,6 +171,8 @@ class DecodeChain:
                 else:
                     self.w[l][i][1].mul_(2.0 ** -20 if not math.isfinite(rms) else 1.0)
                 self._proj(l, i, x, y)
+                if self.tensor_core:
+                    self.gs[l][i].copy_(self.gx)        # the dynamic scale of this input becomes the static one
         torch.cuda.synchronize()
         self.h.copy_(h_bf16)
 

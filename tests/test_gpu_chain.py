@@ -153,3 +153,41 @@ def test_chain_tensor_core_full_size_m8():
         Y, A = orc.gemv_w4a4(hw, hs, np.float32(gw.item()), oxc, oxs, ogx)
         U.check_gemv(U.host_y_f64(y)[:, rows], Y, A, f"full-size tc chain layer {l} {name}")
     assert torch.isfinite(ch.h.float()).all()
+
+
+@pytest.mark.parametrize("M", [1, 8, 24])
+def test_chain_tensor_core_static_scales_fused_quantizers(M):
+    """tensor-core chain with static activation scales: no quantizer launches between projections (each GEMM's epilogue
+    writes the next GEMM's packed NVFP4 input).  Every projection is checked against the oracle: quantize(its BF16 input,
+    static g) -> float64 GEMV on the unpacked weights."""
+    from paper_2606_13233_b200 import binding as B
+    from paper_2606_13233_b200.chain import DecodeChain
+    dims = dict(hidden=512, qkv=768, o_in=512, inter=768)
+    ch = DecodeChain(layers=3, M=M, dims=dims, seed=8, tensor_core=True, static_scales=True)
+    assert ch.launches_per_step == 1 + 5 * 3
+    h0 = U.dev_bf16_from_bits(inputs.make_activation_bits(M, 512, 0, 81))
+    ch.calibrate(h0)
+    taps = []
+    ch.step(taps)
+    torch.cuda.synchronize()
+    assert len(taps) == 12
+    for l, name, x, y in taps:
+        i = [s[0] for s in ch.shapes].index(name)
+        blob, gw, N, K = ch.w[l][i]
+        wc, ws = B.nvfp4_gemm_unpack_weight(blob, N, K)
+        xf = orc.bf16_bits_to_f32(U.host_bf16_bits(x.contiguous()))
+        g_static = np.float32(ch.gs[l][i].item())
+        assert g_static > 0
+        oxc, oxs, ogx = orc.quantize(xf, g=g_static)
+        Y, A = orc.gemv_w4a4(U.host_u8(wc), U.host_u8(ws), np.float32(gw.item()), oxc, oxs, ogx)
+        U.check_gemv(U.host_y_f64(y), Y, A, f"static tc chain layer {l} {name} M={M}", bf16_slack=True)
+    # the timed form (no BF16 outputs between projections) ends on the same bits, eagerly and under graph replay
+    ref = ch.h.clone()
+    ch.set_input(h0); ch.step(); torch.cuda.synchronize()
+    assert torch.equal(ch.h, ref)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        ch.set_input(h0)
+        ch.step()
+    g.replay(); torch.cuda.synchronize()
+    assert torch.equal(ch.h, ref)
