@@ -347,6 +347,21 @@ int nvfp4_gemm_packed_quant_out(const void* w_blob_tc, const float* w_gscale, in
                                 void* xpack_out, const float* out_gscale, int n_quant, void* workspace, size_t ws_bytes,
                                 void* stream);
 
+/*
+ * W4A16 on the tensor cores (BASELINE.json configs[3]: NVFP4 weights, BF16 activations consumed directly, FP32
+ * accumulation), any M >= 1:  Y[M,N] = X_bf16[M,K] . W[N,K]^T  with W in the tensor-core blob of nvfp4_gemm_repack_weight.
+ * The weights are expanded to FP16 in shared memory ONCE per 128-row x 256-k stage (exact: E2M1 value x E4M3 block scale),
+ * whatever M is, and multiplied with the BF16 activations by tcgen05.mma kind::f16 (FP32 accumulator in tensor memory);
+ * the global weight scale is applied in the epilogue.  Same result as nvfp4_gemv(NVFP4_MODE_W4A16) up to FP32 summation
+ * order; acceptance |y - y_ref| <= 1e-3 * sum_k|w_k x_k| + 1e-6.  Deterministic (fixed-order split-K fix-up).
+ *   x_bf16 [M, K] BF16, row stride ldx elements (ldx % 8 == 0, 16-byte aligned rows); K % 256 == 0
+ *   workspace >= nvfp4_gemm_w4a16_workspace_bytes(M, N, K), 16-byte aligned, zero-filled once (counters are left zero)
+ * Launches a small re-layout kernel for the activations and the GEMM per chunk of 32 tokens (W is streamed once per chunk).
+ */
+size_t nvfp4_gemm_w4a16_workspace_bytes(int M, int N, int K);
+int nvfp4_gemm_w4a16(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* x_bf16, int M, int64_t ldx,
+                     void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

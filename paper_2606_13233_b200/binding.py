@@ -30,7 +30,8 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_gemm_repacked_bytes", "nvfp4_gemm_repack_weight", "nvfp4_gemm_unpack_weight",
            "nvfp4_gemm_workspace_bytes", "nvfp4_gemm", "nvfp4_gemm_packed_act_bytes", "nvfp4_gemm_pack_act",
            "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
-           "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc", "nvfp4_gemm_packed_quant_out")
+           "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc", "nvfp4_gemm_packed_quant_out",
+           "nvfp4_gemm_w4a16", "nvfp4_gemm_w4a16_workspace_bytes")
 
 
 class Nvfp4Error(RuntimeError):
@@ -110,6 +111,10 @@ def _load():
     lib.nvfp4_gemm_packed_quant_out.restype = c_int
     lib.nvfp4_gemm_packed_quant_out.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, c_int,
                                                 vp, c_sz, vp]
+    lib.nvfp4_gemm_w4a16_workspace_bytes.restype = c_sz
+    lib.nvfp4_gemm_w4a16_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.nvfp4_gemm_w4a16.restype = c_int
+    lib.nvfp4_gemm_w4a16.argtypes = [vp, vp, c_int, c_int, vp, c_int, c_i64, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_noalloc.restype = c_int
     lib.nvfp4_gemv_noalloc.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp]
     lib.nvfp4_gemm_set_config.restype = c_int
@@ -311,6 +316,18 @@ def nvfp4_gemm_packed_quant_out(w_blob_tc, w_gscale, N, K, xpack, x_gscale, M, o
                                            _ptr(xpack_out), _ptr(out_gscale), n_quant, _ptr(workspace), workspace.numel(),
                                            _stream()))
     return xpack_out, y
+
+
+def nvfp4_gemm_w4a16(w_blob_tc, w_gscale, N, K, x_bf16, y=None, y_dtype=DTYPE_BF16, workspace=None):
+    """tensor-core W4A16 GEMM: NVFP4 weights (tensor-core blob) x BF16 activations [M,K], any M."""
+    M = x_bf16.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=x_bf16.device)
+    if workspace is None:
+        workspace = torch.zeros(max(16, lib.nvfp4_gemm_w4a16_workspace_bytes(M, N, K)), dtype=torch.uint8, device=x_bf16.device)
+    _check(lib.nvfp4_gemm_w4a16(_ptr(w_blob_tc), _ptr(w_gscale), N, K, _ptr(x_bf16), M, x_bf16.stride(0), _ptr(y), y_dtype,
+                                y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
+    return y
 
 
 NOALLOC_SCRATCH_BYTES = 4 << 20

@@ -15,7 +15,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 ROOT = os.path.dirname(PKG)
 LIB = os.path.join(PKG, "libnvfp4_b200.so")
-SOURCES = ["api.cu", "quantize.cu", "repack.cu", "gemv.cu", "gemv_w4a4.cu", "gemv_w4a4h.cu", "gemv_w4a16.cu", "misc.cu", "sampler.cu", "gemm_tc.cu", "noalloc.cu"]
+SOURCES = ["api.cu", "quantize.cu", "repack.cu", "gemv.cu", "gemv_w4a4.cu", "gemv_w4a4h.cu", "gemv_w4a16.cu", "misc.cu", "sampler.cu", "gemm_tc.cu", "gemm_tc16.cu", "noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]        # NOTE: never -use_fast_math (bit-exact quantizer)

@@ -413,4 +413,24 @@ int nvfp4_gemm_packed_quant_out(const void* w_blob_tc, const float* w_gscale, in
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+size_t nvfp4_gemm_w4a16_workspace_bytes(int M, int N, int K) {
+    if (M < 1 || M > (1 << 20) || N < 1 || K < 1 || !gemm_tc_supported(N, K)) return 0;
+    return gemm_tc16_workspace_bytes(M, N, K);
+}
+
+int nvfp4_gemm_w4a16(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* x_bf16, int M, int64_t ldx,
+                     void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+    g_last_err[0] = 0;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob_tc || !w_gscale || !x_bf16 || !y || !workspace) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > (1 << 20) || N < 1 || K < 1 || !gemm_tc_supported(N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (ldy < N || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob_tc) || !aligned16(x_bf16) || !aligned16(y) || !aligned16(workspace) ||
+        (reinterpret_cast<uintptr_t>(w_gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    if (ws_bytes < gemm_tc16_workspace_bytes(M, N, K)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemm_tc16(w_blob_tc, w_gscale, N, K, x_bf16, ldx, M, y, y_dtype, ldy, workspace, ws_bytes,
+                                     static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 }  // extern "C"

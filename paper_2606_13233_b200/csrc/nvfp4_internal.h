@@ -91,4 +91,9 @@ cudaError_t launch_gemm_tc(const void* blob, const float* w_gscale, int N, int K
                            const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, void* y, int y_dtype,
                            int64_t ldy, void* workspace, size_t ws_bytes, cudaStream_t st);
 
+// tensor-core W4A16 GEMM (gemm_tc16.cu): NVFP4 weights in the tensor-core blob, BF16 activations
+size_t gemm_tc16_workspace_bytes(int M, int N, int K);
+cudaError_t launch_gemm_tc16(const void* blob, const float* w_gscale, int N, int K, const void* x_bf16, int64_t ldx, int M,
+                             void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, cudaStream_t st);
+
 }  // namespace nvfp4
