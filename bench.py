@@ -362,10 +362,24 @@ class ShapeBank:
             tcb.append(B.nvfp4_gemm_repack_weight(codes, scales))
             del codes, scales
         out = {}
+        self.w4a16_tc = {}
         for M in Ms:
             xbits = inputs.make_activation_bits(min(M, 8), K, seed=0, shape_id=self.sid)
             x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
             x = x.repeat((M + 7) // 8, 1)[:M].contiguous()
+            if M <= 32:      # W4A16 on the tensor cores (nvfp4_gemm_w4a16: activation re-layout + GEMM), same rotation
+                y16 = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+                ws16 = torch.zeros(B.lib.nvfp4_gemm_w4a16_workspace_bytes(M, N, K), dtype=torch.uint8, device="cuda")
+                call16 = lambda b: B.nvfp4_gemm_w4a16(b, self.gw, N, K, x, y=y16, y_dtype=B.DTYPE_BF16, workspace=ws16)
+                for b in tcb[:2]:
+                    call16(b)
+                torch.cuda.synchronize()
+                g16 = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g16):
+                    for b in tcb:
+                        call16(b)
+                self.w4a16_tc[M] = time_graph(torch, g16, max(3, reps_total // self.copies), 3) / self.copies * 1e3
+                del g16
             xp, gx = B.nvfp4_quantize_act_packed(x)
             y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
             ws = B.nvfp4_gemm_packed_new_workspace(M, N, K, "cuda")
@@ -565,6 +579,9 @@ def run_ours(args):
                 tc_rows.setdefault(str(m), {})[name] = {"us": round(tc[m], 2), "frac": round(nb / tc[m] / 1e3 / peak, 3)}
                 if m in shape_rows:
                     shape_rows[m][name]["tensor_core_us"] = round(tc[m], 2)
+                    shape_rows[m][name]["w4a16_tensor_core_us"] = round(bank.w4a16_tc[m], 2)
+                if m in bank.w4a16_tc:
+                    tc_rows[str(m)][name]["w4a16_us"] = round(bank.w4a16_tc[m], 2)
             wins = [m for m in MS if tc[m] < shape_rows[m][name]["us"]]
             tc_cross[name] = min(wins) if wins else None
             del bank

@@ -5,9 +5,11 @@
 // 2-3x slower than cuBLAS BF16 at M = 8.  Here the per-weight work is done ONCE whatever M is:
 //   * the weights stream from HBM in the tensor-core blob of gemm_tc.cu (0.5625 B per weight, one bulk copy per
 //     128-row x 256-k stage),
-//   * eight "dequant" warps expand a stage to FP16 in shared memory: cvt.rn.f16x2.e2m1x2 (exact) times the block scale as
-//     FP16 (exact: a 2-bit times a 4-bit significand, |value| <= 6 * 448), written as the 8-row x 16-byte core matrices
-//     the MMA reads.  The global weight scale stays out (epilogue),
+//   * sixteen "dequant" warps expand a stage to FP16: cvt.rn.f16x2.e2m1x2 (exact) times the block scale as FP16 (exact: a
+//     2-bit times a 4-bit significand, |value| <= 6 * 448), and write it with tcgen05.st straight into TENSOR MEMORY as the
+//     MMA's A operand (lane = weight row, two FP16 per 32-bit column along k).  A first version kept the FP16 image in
+//     shared memory: every K = 16 MMA then re-read 4 KB of A from shared memory (~90 cycles per MMA, 16 per stage) and
+//     the kernel ran at 0.3 of the copy ceiling.  The global weight scale stays out (epilogue),
 //   * tcgen05.mma kind::f16 with A = those FP16 weights (128 rows = TMEM lanes), B = the activations (tokens = MMA N), FP32
 //     accumulator in tensor memory.  The hardware rejects mixed FP16 x BF16 operands (illegal instruction, measured), and a
 //     BF16 image of the weights costs twice the instructions per weight (there is no e2m1 -> bf16 conversion), so the
@@ -16,6 +18,8 @@
 //     row's maximum is then an FP16 normal, i.e. converted EXACTLY; smaller elements round at 2^-24 * 2^-15 of the row
 //     maximum, below the FP32 accumulator's own resolution (R23).  2^p is multiplied back in the epilogue,
 //   * epilogue: y = acc * gW * 2^p[m], BF16 or FP32.
+// Measured limit: a tcgen05.mma costs ~60 cycles whatever N <= 128 is, and FP16 operands allow only K = 16 per instruction:
+// 16 MMAs = ~1000 cycles per 18 KB stage, i.e. the kernel is MMA-issue bound at ~0.43 of the HBM copy ceiling, flat in M.
 // Work split: items = (tile, K slice), one after the other per persistent CTA; with K slices the partial sums meet in the
 // workspace and the last slice to arrive (per-tile counter) adds them in slice order (deterministic).
 #include "nvfp4_common.cuh"
@@ -24,34 +28,39 @@
 
 namespace nvfp4 {
 
-constexpr int T16_DQ_WARPS  = 8;                       // dequant warps
+constexpr int T16_DQ_WARPS  = 12;                      // dequant warps: three groups of four, group i expands the stages g = i (mod 3) into A buffer i
 constexpr int T16_THREADS   = (6 + T16_DQ_WARPS) * 32; // producer, MMA issuer, 4 epilogue warps, dequant warps
-constexpr int T16_HALF_K    = 128;                     // k expanded per A buffer
-constexpr int T16_ABUF      = TC_TILE_N * T16_HALF_K * 2;   // 32768 B of FP16
+constexpr int T16_ACOLS     = TC_STAGE_K / 2;          // 128 TMEM columns hold one stage of FP16 weights (2 per column)
+constexpr int T16_A0        = 64;                      // first A column (after the two accumulators of <= 32 columns)
+constexpr int T16_NBUF      = 3;                       // A buffers in tensor memory: 64 + 3 * 128 = 448 of the 512 columns
+constexpr int T16_TMEM_COLS = 512;
 constexpr int T16_MAX_MT    = 32;
 constexpr int T16_MAX_CTAS  = 148;
-#ifndef T16_AFMT
-#define T16_AFMT 0u
-#define T16_BFMT 0u
-#endif
 
 __host__ __device__ constexpr int t16_xrec_bytes(int MT) { return MT * TC_STAGE_K * 2; }            // BF16 activations of a stage
 __host__ __device__ constexpr int t16_slot_bytes(int MT) { return TC_STAGE_BYTES + t16_xrec_bytes(MT); }
 __host__ __device__ constexpr int t16_dstride(int MT) { return MT < 32 ? 32 : MT; }
-__host__ __device__ constexpr int t16_tmem_cols(int MT) { return 2 * t16_dstride(MT); }              // 64 (power of two >= 32)
 
 // instruction descriptor of kind::f16: D = F32, A = B = F16 (format 0), both K-major, D = 128 x MT, K = 16
 __host__ __device__ constexpr uint32_t t16_idesc(int MT) {
-    return (1u << 4) | (T16_AFMT << 7) | (T16_BFMT << 10) | ((uint32_t)(MT >> 3) << 17) | ((uint32_t)(TC_TILE_N >> 4) << 24);
+    return (1u << 4) | (0u << 7) | (0u << 10) | ((uint32_t)(MT >> 3) << 17) | ((uint32_t)(TC_TILE_N >> 4) << 24);
 }
-__device__ __forceinline__ void tc_mma_f16(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+// A from tensor memory, B from shared memory
+__device__ __forceinline__ void tc_mma_f16_ts(uint32_t d, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
-        "}\n" ::"r"(d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(d), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// this thread's TMEM lane, 16 consecutive 32-bit columns
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+                   "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // ---- activations: BF16 X[M,K] (row stride ldx elements) -> FP16, per 256-k stage the MMA's B image: 8-token x 16-byte
 // core matrices, chunk kc8 (8 k) of token t at (kc8*(MT/8) + t/8)*128 + (t%8)*16; tokens >= M are zero.
@@ -142,9 +151,11 @@ __device__ __forceinline__ uint32_t t16_prmt(uint32_t a, uint32_t b, uint32_t se
     return d;
 }
 // eight E2M1 codes (one 32-bit word, low nibble first) times an FP16 scale pair {s, s} -> eight FP16 (exact)
-__device__ __forceinline__ uint4 t16_expand8(uint32_t w, uint32_t s2) {
-    return make_uint4(t16_hmul2(e2m1x2_to_f16x2(w & 0xFFu), s2), t16_hmul2(e2m1x2_to_f16x2((w >> 8) & 0xFFu), s2),
-                      t16_hmul2(e2m1x2_to_f16x2((w >> 16) & 0xFFu), s2), t16_hmul2(e2m1x2_to_f16x2(w >> 24), s2));
+__device__ __forceinline__ void t16_expand8(uint32_t w, uint32_t s2, uint32_t* out) {
+    out[0] = t16_hmul2(e2m1x2_to_f16x2(w & 0xFFu), s2);
+    out[1] = t16_hmul2(e2m1x2_to_f16x2((w >> 8) & 0xFFu), s2);
+    out[2] = t16_hmul2(e2m1x2_to_f16x2((w >> 16) & 0xFFu), s2);
+    out[3] = t16_hmul2(e2m1x2_to_f16x2(w >> 24), s2);
 }
 __device__ __forceinline__ void t16_epi_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }   // the 4 epilogue warps
 
@@ -154,12 +165,11 @@ __global__ void __launch_bounds__(T16_THREADS, 1) gemm_tc16_kernel(const Gemm16P
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int S = p.stages;
     constexpr int SLOT = t16_slot_bytes(MT), XREC = t16_xrec_bytes(MT);
-    constexpr int DSTRIDE = t16_dstride(MT), NCOLS = t16_tmem_cols(MT);
+    constexpr int DSTRIDE = t16_dstride(MT), NCOLS = T16_TMEM_COLS;
     uint8_t* ring = smem;
-    uint8_t* abuf = smem + (size_t)S * SLOT;                                  // 2 x T16_ABUF
-    uint64_t* bars = reinterpret_cast<uint64_t*>(abuf + 2 * T16_ABUF);
-    uint64_t *full = bars, *empty = bars + S, *afull = bars + 2 * S, *aempty = afull + 2, *tfull = afull + 4, *tempty = afull + 6;
-    volatile uint32_t* misc = reinterpret_cast<volatile uint32_t*>(afull + 8);       // [0] TMEM base [1] last [2] blob ok
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)S * SLOT);
+    uint64_t *full = bars, *empty = bars + S, *afull = bars + 2 * S, *aempty = afull + T16_NBUF, *tfull = afull + 2 * T16_NBUF, *tempty = tfull + 2;
+    volatile uint32_t* misc = reinterpret_cast<volatile uint32_t*>(tempty + 2);       // [0] TMEM base [1] last [2] blob ok
 
     const int KS = p.KS, ksplit = p.ksplit, items = p.T * ksplit;
     auto item_range = [&](int item, int& tile, int& slice, int& k0, int& k1) {
@@ -178,10 +188,8 @@ __global__ void __launch_bounds__(T16_THREADS, 1) gemm_tc16_kernel(const Gemm16P
         npre = k1 - k0 < S ? k1 - k0 : S;
         if (threadIdx.x == 0) {
             for (int i = 0; i < S; ++i) { mbar_init(smem_u32(full + i), 1); mbar_init(smem_u32(empty + i), 1); }
-            for (int i = 0; i < 2; ++i) {
-                mbar_init(smem_u32(afull + i), T16_DQ_WARPS); mbar_init(smem_u32(aempty + i), 1);
-                mbar_init(smem_u32(tfull + i), 1); mbar_init(smem_u32(tempty + i), 4);
-            }
+            for (int i = 0; i < T16_NBUF; ++i) { mbar_init(smem_u32(afull + i), 4); mbar_init(smem_u32(aempty + i), 1); }
+            for (int i = 0; i < 2; ++i) { mbar_init(smem_u32(tfull + i), 1); mbar_init(smem_u32(tempty + i), 4); }
             mbar_fence_init();
             for (int i = 0; i < npre; ++i) {
                 mbar_arrive_expect_tx(smem_u32(full + i), (uint32_t)SLOT);
@@ -226,8 +234,8 @@ __global__ void __launch_bounds__(T16_THREADS, 1) gemm_tc16_kernel(const Gemm16P
         constexpr uint32_t IDESC = t16_idesc(MT);
         constexpr uint32_t B_LBO = (MT / 8) * 128;
         constexpr uint32_t HI = (128u >> 4) | (1u << 14);                                 // SBO = 128 | descriptor version 1
-        constexpr uint32_t A_LO = (2048u >> 4) << 16, B_LO = (B_LBO >> 4) << 16;        // LBO
-        const uint32_t ring0 = smem_u32(ring), a0 = smem_u32(abuf) >> 4;
+        constexpr uint32_t B_LO = (B_LBO >> 4) << 16;                                     // LBO
+        const uint32_t ring0 = smem_u32(ring);
         const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty), afull0 = smem_u32(afull), aempty0 = smem_u32(aempty);
         const uint32_t tfull0 = smem_u32(tfull), tempty0 = smem_u32(tempty);
         int g = 0, il = 0;
@@ -240,66 +248,76 @@ __global__ void __launch_bounds__(T16_THREADS, 1) gemm_tc16_kernel(const Gemm16P
             const uint32_t d = tbase + (uint32_t)ab * DSTRIDE;
             uint32_t acc = 0;
             for (int k = k0; k < k1; ++k, ++g) {
-                const int slot = g % S, use = g / S;
-                mbar_wait(full0 + 8u * slot, (uint32_t)(use & 1));                      // the stage's BF16 activations have landed
+                const int slot = g % S, use = g / S, buf = g % T16_NBUF, bround = g / T16_NBUF;
+                mbar_wait(full0 + 8u * slot, (uint32_t)(use & 1));                      // the stage's activations have landed
+                mbar_wait(afull0 + 8u * buf, (uint32_t)(bround & 1));                 // its FP16 weights are in tensor memory
+                tc_fence_after();
                 const uint32_t xb = (ring0 + (uint32_t)slot * SLOT + TC_STAGE_BYTES) >> 4;
+                const uint32_t at = tbase + T16_A0 + (uint32_t)buf * T16_ACOLS;
+                if (elected) {
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    mbar_wait(afull0 + 8u * h, (uint32_t)(g & 1));                      // FP16 weights of this half are in place
-                    tc_fence_after();
-                    if (elected) {
-#pragma unroll
-                        for (int j = 0; j < T16_HALF_K / 16; ++j) {
-#ifndef T16_EXP_NOMMA
-                            tc_mma_f16(d, tc_desc((a0 + (uint32_t)((h * T16_ABUF + j * 2 * 2048) >> 4)) | A_LO, HI),
-                                       tc_desc((xb + (uint32_t)(((h * 16 + j * 2) * B_LBO) >> 4)) | B_LO, HI), IDESC, acc);
-#endif
-                            acc = 1;
-                        }
-                        tc_commit(aempty0 + 8u * h);          // the dequant warps may refill this half
-                        if (h == 1) tc_commit(empty0 + 8u * slot);                      // and the producer the ring slot
+                    for (int j = 0; j < TC_STAGE_K / 16; ++j) {
+                        tc_mma_f16_ts(d, at + 8u * j, tc_desc((xb + (uint32_t)((j * 2 * B_LBO) >> 4)) | B_LO, HI), IDESC, acc);
+                        acc = 1;
                     }
-                    acc = 1;
+                    tc_commit(aempty0 + 8u * buf);            // the dequant warps may refill this A buffer
+                    tc_commit(empty0 + 8u * slot);            // and the producer the ring slot
                 }
+                acc = 1;
             }
             if (elected) tc_commit(tfull0 + 8u * ab);
         }
         __syncwarp();
     } else if (warp >= 6) {                                   // ---- dequant warps ----
-        const int dw = warp - 6;
+        // a warp can only reach the 32 TMEM lanes of its quarter (warp % 4): it expands those 32 weight rows, all 256 k of a
+        // stage.  Three groups of four warps take the stages round-robin, group i always into A buffer i: a warp works
+        // through its stages one after the other (wait, load, convert, tcgen05.st, wait::st, arrive), so several stages must
+        // be in expansion at any time; three A buffers are what fits into tensor memory.  (One group per buffer also keeps
+        // every mbarrier wait within one phase of the barrier: a group that could run two buffer generations ahead of the
+        // MMAs would see the parity of an older phase and pass -- measured as an intermittent deadlock.)
+        const int dw = warp - 6, grp = dw >> 2, rg = warp & 3, r = rg * 32 + lane;
+        constexpr int NGRP = T16_DQ_WARPS / 4;
+        static_assert(NGRP == T16_NBUF, "one dequant group per A buffer");
         const uint32_t full0 = smem_u32(full), afull0 = smem_u32(afull), aempty0 = smem_u32(aempty);
+        const uint32_t tlane = tbase + ((uint32_t)(rg * 32) << 16) + T16_A0;
         int g = 0;
         for (int item = blockIdx.x; item < items; item += gridDim.x) {
             int tile, slice, k0, k1;
             item_range(item, tile, slice, k0, k1);
             for (int k = k0; k < k1; ++k, ++g) {
-                const int slot = g % S, use = g / S;
+                if (g % NGRP != grp) continue;
+                const int slot = g % S, use = g / S, buf = g % T16_NBUF, bround = g / T16_NBUF;
                 mbar_wait(full0 + 8u * slot, (uint32_t)(use & 1));
                 const uint8_t* st = ring + (size_t)slot * SLOT;
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    if (g >= 1) mbar_wait(aempty0 + 8u * h, (uint32_t)((g - 1) & 1));
-                    uint8_t* ah = abuf + (size_t)h * T16_ABUF;
+                for (int b4 = 0; b4 < 2; ++b4) {              // the quarter's eight 32-k chunks in two batches of four
+                    uint4 cw[4];
+                    uint16_t sc2[4];
 #pragma unroll
-                    for (int it = 0; it < 2; ++it) {
-                        const int u = it * T16_DQ_WARPS + dw, rg = u & 3, kcl = u >> 2;  // 4 row groups x 4 chunks of 32 k
-                        const int kc = h * 4 + kcl, r = rg * 32 + lane;
-                        const uint4 cw = *reinterpret_cast<const uint4*>(st + (size_t)((kc * 16 + (r >> 3)) * 128 + (r & 7) * 16));
-                        const uint16_t sc2 = *reinterpret_cast<const uint16_t*>(st + TC_CODE_BYTES + (kc >> 1) * 512 + (r & 31) * 16 +
-                                                                                 (r >> 5) * 4 + (kc & 1) * 2);
-                        uint32_t s2;
-                        asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(s2) : "h"(sc2));
-                        const uint32_t sA = t16_prmt(s2, s2, 0x1010u), sB = t16_prmt(s2, s2, 0x3232u);
-                        uint4* dst = reinterpret_cast<uint4*>(ah + (size_t)((kcl * 4 * 16 + (r >> 3)) * 128 + (r & 7) * 16));
-                        dst[0 * 16 * 8] = t16_expand8(cw.x, sA);                        // k-chunk stride = 16 row groups x 128 B
-                        dst[1 * 16 * 8] = t16_expand8(cw.y, sA);
-                        dst[2 * 16 * 8] = t16_expand8(cw.z, sB);
-                        dst[3 * 16 * 8] = t16_expand8(cw.w, sB);
+                    for (int i = 0; i < 4; ++i) {             // all loads first: the expansion is latency bound
+                        const int kc = b4 * 4 + i;
+                        cw[i] = *reinterpret_cast<const uint4*>(st + (size_t)((kc * 16 + (r >> 3)) * 128 + (r & 7) * 16));
+                        sc2[i] = *reinterpret_cast<const uint16_t*>(st + TC_CODE_BYTES + (kc >> 1) * 512 + (r & 31) * 16 + (r >> 5) * 4 + (kc & 1) * 2);
                     }
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");        // generic stores -> the MMA's async reads
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_plain(afull0 + 8u * h);
+                    if (b4 == 0) {
+                        if (bround >= 1) mbar_wait(aempty0 + 8u * buf, (uint32_t)((bround - 1) & 1));   // the MMAs that read this buffer are done
+                        tc_fence_after();
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        uint32_t s2;
+                        asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(s2) : "h"(sc2[i]));
+                        const uint32_t sA = t16_prmt(s2, s2, 0x1010u), sB = t16_prmt(s2, s2, 0x3232u);
+                        uint32_t v[16];
+                        t16_expand8(cw[i].x, sA, v); t16_expand8(cw[i].y, sA, v + 4);
+                        t16_expand8(cw[i].z, sB, v + 8); t16_expand8(cw[i].w, sB, v + 12);
+                        tmem_st16(tlane + (uint32_t)buf * T16_ACOLS + (uint32_t)(b4 * 4 + i) * 16, v);
+                    }
                 }
+                tmem_st_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_plain(afull0 + 8u * buf);
             }
         }
     } else {                                                  // ---- epilogue (warps 2..5) ----
@@ -376,7 +394,7 @@ __global__ void __launch_bounds__(T16_THREADS, 1) gemm_tc16_kernel(const Gemm16P
 // kind::f16 with 128 accumulator rows needs N % 16 == 0 (N = 8 traps as an illegal instruction): 16 token columns at least
 static int t16_pick_mt(int m) { return m <= 16 ? 16 : 32; }
 static int t16_pick_stages(int MT) {
-    const int s = (227 * 1024 - 2 * T16_ABUF - 512) / t16_slot_bytes(MT);
+    const int s = (227 * 1024 - 512) / t16_slot_bytes(MT);
     return s > 8 ? 8 : s;
 }
 // K slices per tile and persistent CTAs: as for the W4A4 tensor-core kernel (tc_pick_ctas), items are whole K slices of
@@ -411,7 +429,7 @@ size_t gemm_tc16_workspace_bytes(int M, int N, int K) {
 template <int MT>
 static cudaError_t launch_gemm_tc16_mt(const Gemm16Params& p, int grid, cudaStream_t st) {
     static size_t configured[MAX_DEVICES] = {};
-    const size_t smem = (size_t)p.stages * t16_slot_bytes(MT) + 2 * T16_ABUF + (size_t)(2 * p.stages + 8) * 8 + 32;
+    const size_t smem = (size_t)p.stages * t16_slot_bytes(MT) + (size_t)(2 * p.stages + 2 * T16_NBUF + 4) * 8 + 32;
     cudaError_t e = ensure_dynamic_smem(gemm_tc16_kernel<MT>, configured, smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};

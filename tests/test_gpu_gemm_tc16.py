@@ -108,3 +108,24 @@ def test_strided_activations_and_wrong_blob(B):
     U.check_gemv(U.host_y_f64(y), c["Y"], c["A"], "strided x")
     blob[8] ^= 1
     assert torch.isnan(B.nvfp4_gemm_w4a16(blob, U.dev_f32(c["gw"]), N, K, big[:, :K], y_dtype=B.DTYPE_F32)).all()
+
+
+def test_many_back_to_back_launches_do_not_deadlock_or_drift(B):
+    """regression for an intermittent deadlock (a dequant group running two buffer generations ahead of the MMAs passed an
+    mbarrier wait on the parity of an older phase): hundreds of launches back to back, graph replayed, identical bits."""
+    for M, N, K in [(4, 10240, 5120), (7, 5120, 8192)]:
+        codes, scales, _ = inputs.make_nvfp4_weight_device(N, K, seed=1, shape_id=1)
+        blob = B.nvfp4_gemm_repack_weight(codes, scales)
+        gw = U.dev_f32(3e-5)
+        x = U.dev_bf16_from_bits(inputs.make_activation_bits(M, K, 0, 1))
+        ws = torch.zeros(B.lib.nvfp4_gemm_w4a16_workspace_bytes(M, N, K), dtype=torch.uint8, device="cuda")
+        y0 = B.nvfp4_gemm_w4a16(blob, gw, N, K, x, y_dtype=B.DTYPE_BF16, workspace=ws).clone()
+        y = torch.empty_like(y0)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for _ in range(20):
+                B.nvfp4_gemm_w4a16(blob, gw, N, K, x, y=y, y_dtype=B.DTYPE_BF16, workspace=ws)
+        for _ in range(15):
+            g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(y, y0)
