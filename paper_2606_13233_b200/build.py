@@ -21,8 +21,6 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]        # NOTE: never -use_fast_math (bit-exact quantizer)
 if os.environ.get("NVFP4_ENABLE_TRACE"):                 # debug builds: %globaltimer stamps in the GEMV (nvfp4_debug_set_trace)
     FLAGS.append("-DNVFP4_ENABLE_TRACE")
-if os.environ.get("NVFP4_TC_EXP"):
-    FLAGS.append("-D" + os.environ["NVFP4_TC_EXP"])
 
 
 def _deps():

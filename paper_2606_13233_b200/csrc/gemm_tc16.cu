@@ -18,8 +18,11 @@
 //     row's maximum is then an FP16 normal, i.e. converted EXACTLY; smaller elements round at 2^-24 * 2^-15 of the row
 //     maximum, below the FP32 accumulator's own resolution (R23).  2^p is multiplied back in the epilogue,
 //   * epilogue: y = acc * gW * 2^p[m], BF16 or FP32.
-// Measured limit: a tcgen05.mma costs ~60 cycles whatever N <= 128 is, and FP16 operands allow only K = 16 per instruction:
-// 16 MMAs = ~1000 cycles per 18 KB stage, i.e. the kernel is MMA-issue bound at ~0.43 of the HBM copy ceiling, flat in M.
+// Measured limit: with a handful of token columns the tensor core cannot reuse the A operand, and it takes A in at ~64 B per
+// clock: a K = 16 FP16 MMA (4 KB of A) costs ~62 cycles whatever N is (independent accumulators do not help, A from
+// shared memory costs ~88), i.e. ~1000 cycles per 128 x 256 stage against the ~830 cycles the stage's 18 KB take to arrive
+// from HBM: the kernel is A-feed bound at ~0.43 of the copy ceiling, flat in M up to 32.  (The W4A4 kernel's FP4 A
+// operand is four times smaller: 4 MMAs x 64 cycles per stage, which is why it stays on the HBM roofline.)
 // Work split: items = (tile, K slice), one after the other per persistent CTA; with K slices the partial sums meet in the
 // workspace and the last slice to arrive (per-tile counter) adds them in slice order (deterministic).
 #include "nvfp4_common.cuh"
