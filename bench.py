@@ -119,7 +119,7 @@ class Workload:
             blobs = []
             for c in range(copies):
                 codes, scales, g = inputs.make_nvfp4_weight_device(N, K, seed=c, shape_id=sid)
-                blobs.append(B.nvfp4_gemm_repack_weight(codes, scales) if mode == "tc" else B.nvfp4_repack_weight(codes, scales))
+                blobs.append(B.nvfp4_gemm_repack_weight(codes, scales) if mode in ("tc", "w4a16tc") else B.nvfp4_repack_weight(codes, scales))
                 del codes, scales
             xbits = inputs.make_activation_bits(M, K, seed=0, shape_id=sid)
             x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
@@ -132,7 +132,9 @@ class Workload:
                 gx=torch.zeros(1, dtype=torch.float32, device="cuda"),
                 y=torch.empty((M, N), dtype=torch.bfloat16, device="cuda"),
                 xp=(torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device="cuda") if mode == "tc" else None),
-                ws=(B.nvfp4_gemm_packed_new_workspace(M, N, K, "cuda") if mode == "tc" else B.new_workspace(M, N, K))))
+                ws=(B.nvfp4_gemm_packed_new_workspace(M, N, K, "cuda") if mode == "tc" else
+                    torch.zeros(B.lib.nvfp4_gemm_w4a16_workspace_bytes(M, N, K), dtype=torch.uint8, device="cuda") if mode == "w4a16tc"
+                    else B.new_workspace(M, N, K))))
         # e2e staging: the step's four activations / outputs as ONE pinned host buffer and ONE device buffer each
         # (element offsets are multiples of 8 BF16 = 16 B), so a step costs one H2D and one D2H copy
         def pack(key, host_key):
@@ -163,6 +165,8 @@ class Workload:
         if self.mode == "tc":          # the tcgen05 GEMM on packed activations
             B.nvfp4_gemm_packed(p["blobs"][copy], p["gw"], p["N"], p["K"], p["xp"], p["gx"], self.M, y=p["y"],
                                 y_dtype=B.DTYPE_BF16, workspace=p["ws"])
+        elif self.mode == "w4a16tc":   # W4A16 on the tensor cores (activation re-layout + GEMM)
+            B.nvfp4_gemm_w4a16(p["blobs"][copy], p["gw"], p["N"], p["K"], p["x"], y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
         elif self.mode == "w4a4":
             B.nvfp4_gemv(B.MODE_W4A4, p["blobs"][copy], p["gw"], p["N"], p["K"], p["xc"], p["xs"], p["gx"],
                          y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
@@ -808,7 +812,7 @@ def main():
     ap.add_argument("--headline-only", action="store_true", help="only the configs[1] step at --m rows (no per_m table)")
     ap.add_argument("--profile-shape", default=None, help="qkv|o|gate_up|down|all: plain stream launches of "
                     "quantize_act + gemv on that shape only (for ncu); prints a short JSON line")
-    ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16", "tc"], help="profile leg: CUDA-core W4A4 / W4A16 GEMV, or tc = the tcgen05 GEMM path")
+    ap.add_argument("--mode", default="w4a4", choices=["w4a4", "w4a16", "tc", "w4a16tc"], help="profile leg: CUDA-core W4A4 / W4A16 GEMV, tc = the tcgen05 W4A4 GEMM path, w4a16tc = the tensor-core W4A16 GEMM")
     ap.add_argument("--chain", action="store_true", help="configs[4]: decode-step projection chain, M = 1,2,4,8")
     ap.add_argument("--layers", type=int, default=64)
     args = ap.parse_args()

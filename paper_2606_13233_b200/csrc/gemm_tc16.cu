@@ -155,10 +155,10 @@ __device__ __forceinline__ uint32_t t16_prmt(uint32_t a, uint32_t b, uint32_t se
 }
 // eight E2M1 codes (one 32-bit word, low nibble first) times an FP16 scale pair {s, s} -> eight FP16 (exact)
 __device__ __forceinline__ void t16_expand8(uint32_t w, uint32_t s2, uint32_t* out) {
-    out[0] = t16_hmul2(e2m1x2_to_f16x2(w & 0xFFu), s2);
-    out[1] = t16_hmul2(e2m1x2_to_f16x2((w >> 8) & 0xFFu), s2);
-    out[2] = t16_hmul2(e2m1x2_to_f16x2((w >> 16) & 0xFFu), s2);
-    out[3] = t16_hmul2(e2m1x2_to_f16x2(w >> 24), s2);
+    uint32_t h[4];
+    cvt_word_e2m1(w, h);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) out[i] = t16_hmul2(h[i], s2);
 }
 __device__ __forceinline__ void t16_epi_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }   // the 4 epilogue warps
 

@@ -172,10 +172,12 @@ __device__ __forceinline__ void decode_x_block(uint2 cw, float sx, uint8_t* base
 // FP16 variant of the record: 16 e2m1 values as f16 (8 x F2FP), the block scale as FP32
 __device__ __forceinline__ void decode_x_block_h(uint2 cw, float sx, uint8_t* base, int half) {
     uint32_t h[8];
+    {
+        uint32_t a[4], b[4];
+        cvt_word_e2m1(cw.x, a);
+        cvt_word_e2m1(cw.y, b);
 #pragma unroll
-    for (int b = 0; b < 4; ++b) {
-        h[b]     = e2m1x2_to_f16x2((cw.x >> (8 * b)) & 0xFFu);
-        h[4 + b] = e2m1x2_to_f16x2((cw.y >> (8 * b)) & 0xFFu);
+        for (int i = 0; i < 4; ++i) { h[i] = a[i]; h[4 + i] = b[i]; }
     }
     uint4* dst = reinterpret_cast<uint4*>(base + half * 32);
     dst[0] = make_uint4(h[0], h[1], h[2], h[3]);
@@ -401,11 +403,6 @@ __device__ __forceinline__ uint32_t hadd2(uint32_t a, uint32_t b) {
     asm("add.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
     return d;
 }
-__device__ __forceinline__ void cvt_word_e2m1(uint32_t w, uint32_t (&h)[4]) {
-    asm("{.reg .b8 t0,t1,t2,t3; mov.b32 {t0,t1,t2,t3}, %4;\n"
-        "cvt.rn.f16x2.e2m1x2 %0, t0; cvt.rn.f16x2.e2m1x2 %1, t1; cvt.rn.f16x2.e2m1x2 %2, t2; cvt.rn.f16x2.e2m1x2 %3, t3;}"
-        : "=r"(h[0]), "=r"(h[1]), "=r"(h[2]), "=r"(h[3]) : "r"(w));
-}
 __device__ __forceinline__ float2 h2_to_float2(uint32_t h2) {
     float2 r;
     asm("{.reg .b16 lo, hi; mov.b32 {lo, hi}, %2; cvt.f32.f16 %0, lo; cvt.f32.f16 %1, hi;}"
@@ -484,12 +481,15 @@ __device__ __forceinline__ void block_pair_w4a16(const uint4 (&wv)[R], const uin
         for (int h = 0; h < 2; ++h) {                                      // the two 16-blocks
             uint64_t wp[8];
 #pragma unroll
-            for (int q = 0; q < 2; ++q)
+            for (int q = 0; q < 2; ++q) {
+                uint32_t hw[4];
+                cvt_word_e2m1(ww[h * 2 + q], hw);
 #pragma unroll
                 for (int b = 0; b < 4; ++b) {
-                    const float2 f = h2_to_float2(e2m1x2_to_f16x2((ww[h * 2 + q] >> (8 * b)) & 0xFFu));
+                    const float2 f = h2_to_float2(hw[b]);
                     wp[q * 4 + b] = pack2(f.x, f.y);
                 }
+            }
 #pragma unroll
             for (int m = 0; m < M; ++m) {
                 const ulonglong2* xp = reinterpret_cast<const ulonglong2*>(xbp + m * XBP_W4A16) + h * 4;

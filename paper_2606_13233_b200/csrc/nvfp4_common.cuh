@@ -133,6 +133,14 @@ __device__ __forceinline__ uint32_t e2m1x2_to_f16x2(uint32_t byte) {
     return r;
 }
 
+// one 32-bit word of eight E2M1 codes -> four f16x2 (codes 0,1 | 2,3 | 4,5 | 6,7), exact.  The vector mov lets the
+// conversions take their source byte through the instruction's byte selector (F2FP ... R.B1): no shift / mask per byte.
+__device__ __forceinline__ void cvt_word_e2m1(uint32_t w, uint32_t (&h)[4]) {
+    asm("{.reg .b8 t0,t1,t2,t3; mov.b32 {t0,t1,t2,t3}, %4;\n"
+        "cvt.rn.f16x2.e2m1x2 %0, t0; cvt.rn.f16x2.e2m1x2 %1, t1; cvt.rn.f16x2.e2m1x2 %2, t2; cvt.rn.f16x2.e2m1x2 %3, t3;}"
+        : "=r"(h[0]), "=r"(h[1]), "=r"(h[2]), "=r"(h[3]) : "r"(w));
+}
+
 __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) {
     return __uint_as_float(((uint32_t)b) << 16);
 }
