@@ -5,7 +5,7 @@
 // 2-3x slower than cuBLAS BF16 at M = 8.  Here the per-weight work is done ONCE whatever M is:
 //   * the weights stream from HBM in the tensor-core blob of gemm_tc.cu (0.5625 B per weight, one bulk copy per
 //     128-row x 256-k stage),
-//   * sixteen "dequant" warps expand a stage to FP16: cvt.rn.f16x2.e2m1x2 (exact) times the block scale as FP16 (exact: a
+//   * twelve "dequant" warps expand a stage to FP16: cvt.rn.f16x2.e2m1x2 (exact) times the block scale as FP16 (exact: a
 //     2-bit times a 4-bit significand, |value| <= 6 * 448), and write it with tcgen05.st straight into TENSOR MEMORY as the
 //     MMA's A operand (lane = weight row, two FP16 per 32-bit column along k).  A first version kept the FP16 image in
 //     shared memory: every K = 16 MMA then re-read 4 KB of A from shared memory (~90 cycles per MMA, 16 per stage) and
@@ -21,7 +21,7 @@
 // Measured limit: with a handful of token columns the tensor core cannot reuse the A operand, and it takes A in at ~64 B per
 // clock: a K = 16 FP16 MMA (4 KB of A) costs ~62 cycles whatever N is (independent accumulators do not help, A from
 // shared memory costs ~88), i.e. ~1000 cycles per 128 x 256 stage against the ~830 cycles the stage's 18 KB take to arrive
-// from HBM: the kernel is A-feed bound at ~0.43 of the copy ceiling, flat in M up to 32.  (The W4A4 kernel's FP4 A
+// from HBM: the kernel is A-feed bound at 0.32-0.55 of the copy ceiling (gate_up 42 us), flat in M up to 32.  (The W4A4 kernel's FP4 A
 // operand is four times smaller: 4 MMAs x 64 cycles per stage, which is why it stays on the HBM roofline.)
 // Work split: items = (tile, K slice), one after the other per persistent CTA; with K slices the partial sums meet in the
 // workspace and the last slice to arrive (per-tile counter) adds them in slice order (deterministic).
