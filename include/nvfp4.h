@@ -362,6 +362,29 @@ size_t nvfp4_gemm_w4a16_workspace_bytes(int M, int N, int K);
 int nvfp4_gemm_w4a16(const void* w_blob_tc, const float* w_gscale, int N, int K, const void* x_bf16, int M, int64_t ldx,
                      void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream);
 
+/*
+ * The gate_up projection with SiLU * mul AND the down projection's STATIC-scale quantizer in its epilogue (SURVEY.md
+ * 8(f) item 1, step a8 fused): no BF16 gate_up output, no separate SiLU * mul / quantizer launch.
+ *   nvfp4_gemm_repack_weight_gate_up   the tensor-core blob of the fused gate_up weight [N = 2I, K] (gate = rows [0, I),
+ *                                      up = rows [I, 2I), R11) with the rows INTERLEAVED per 128-row tile: 64
+ *                                      gate rows followed by the 64 matching up rows, so one tile owns both factors.
+ *                                      N % 128 == 0; same size as nvfp4_gemm_repacked_bytes(N, K); the header records
+ *                                      the interleaving (a plain nvfp4_gemm on this blob, or this call on a plain blob,
+ *                                      writes NaN).  nvfp4_gemm_unpack_weight_gate_up is its exact inverse.
+ *   nvfp4_gemm_packed_silu_quant_out   h[m, j] = RN_bf16(silu(RN_bf16(gate[m, j])) * RN_bf16(up[m, j])), j < I = N/2 (the
+ *                                      arithmetic of nvfp4_silu_mul on the BF16 GEMM output), quantised with the STATIC
+ *                                      global scale *out_gscale into packed activation records for a following
+ *                                      nvfp4_gemm_packed with K = I (I % 256 == 0): byte-identical to
+ *                                      nvfp4_silu_mul_quantize_packed(STATIC) applied to the plain GEMM's BF16 output.
+ *                                      h_opt (optional, [M, I], row stride ldh) receives h.  Other arguments as for
+ *                                      nvfp4_gemm_packed_quant_out.
+ */
+int nvfp4_gemm_repack_weight_gate_up(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream);
+int nvfp4_gemm_unpack_weight_gate_up(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, void* stream);
+int nvfp4_gemm_packed_silu_quant_out(const void* w_blob_gate_up, const float* w_gscale, int N, int K, const void* xpack,
+                                     const float* x_gscale, int gscale_per_row, int M, void* h_opt, int h_dtype, int64_t ldh,
+                                     void* xpack_out, const float* out_gscale, void* workspace, size_t ws_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

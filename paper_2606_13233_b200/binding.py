@@ -31,7 +31,8 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_gemm_workspace_bytes", "nvfp4_gemm", "nvfp4_gemm_packed_act_bytes", "nvfp4_gemm_pack_act",
            "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
            "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc", "nvfp4_gemm_packed_quant_out",
-           "nvfp4_gemm_w4a16", "nvfp4_gemm_w4a16_workspace_bytes")
+           "nvfp4_gemm_w4a16", "nvfp4_gemm_w4a16_workspace_bytes", "nvfp4_gemm_repack_weight_gate_up",
+           "nvfp4_gemm_unpack_weight_gate_up", "nvfp4_gemm_packed_silu_quant_out")
 
 
 class Nvfp4Error(RuntimeError):
@@ -115,6 +116,12 @@ def _load():
     lib.nvfp4_gemm_w4a16_workspace_bytes.argtypes = [c_int, c_int, c_int]
     lib.nvfp4_gemm_w4a16.restype = c_int
     lib.nvfp4_gemm_w4a16.argtypes = [vp, vp, c_int, c_int, vp, c_int, c_i64, vp, c_int, c_i64, vp, c_sz, vp]
+    lib.nvfp4_gemm_repack_weight_gate_up.restype = c_int
+    lib.nvfp4_gemm_repack_weight_gate_up.argtypes = [vp, vp, c_int, c_int, vp, vp]
+    lib.nvfp4_gemm_unpack_weight_gate_up.restype = c_int
+    lib.nvfp4_gemm_unpack_weight_gate_up.argtypes = [vp, c_int, c_int, vp, vp, vp]
+    lib.nvfp4_gemm_packed_silu_quant_out.restype = c_int
+    lib.nvfp4_gemm_packed_silu_quant_out.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, vp, c_sz, vp]
     lib.nvfp4_gemv_noalloc.restype = c_int
     lib.nvfp4_gemv_noalloc.argtypes = [c_int, vp, vp, c_int, c_int, vp, vp, vp, c_int, c_i64, vp, c_int, c_i64, vp]
     lib.nvfp4_gemm_set_config.restype = c_int
@@ -328,6 +335,34 @@ def nvfp4_gemm_w4a16(w_blob_tc, w_gscale, N, K, x_bf16, y=None, y_dtype=DTYPE_BF
     _check(lib.nvfp4_gemm_w4a16(_ptr(w_blob_tc), _ptr(w_gscale), N, K, _ptr(x_bf16), M, x_bf16.stride(0), _ptr(y), y_dtype,
                                 y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
     return y
+
+
+def nvfp4_gemm_repack_weight_gate_up(codes, scales):
+    """fused gate_up weight [2I, K] -> tensor-core blob with gate / up rows interleaved per tile (see include/nvfp4.h)."""
+    N, K = codes.shape[0], codes.shape[1] * 2
+    blob = torch.empty(lib.nvfp4_gemm_repacked_bytes(N, K), dtype=torch.uint8, device=codes.device)
+    _check(lib.nvfp4_gemm_repack_weight_gate_up(_ptr(codes), _ptr(scales), N, K, _ptr(blob), _stream()))
+    return blob
+
+
+def nvfp4_gemm_unpack_weight_gate_up(blob, N, K):
+    codes = torch.zeros((N, K // 2), dtype=torch.uint8, device=blob.device)
+    scales = torch.zeros((N, K // 16), dtype=torch.uint8, device=blob.device)
+    _check(lib.nvfp4_gemm_unpack_weight_gate_up(_ptr(blob), N, K, _ptr(codes), _ptr(scales), _stream()))
+    return codes, scales
+
+
+def nvfp4_gemm_packed_silu_quant_out(w_blob_gate_up, w_gscale, N, K, xpack, x_gscale, M, out_gscale, xpack_out=None, h=None,
+                                     h_dtype=DTYPE_BF16, workspace=None, gscale_per_row=False):
+    """gate_up GEMM + SiLU*mul + STATIC-scale quantizer in one launch: packed records of h [M, N/2] for the down GEMM."""
+    if xpack_out is None:
+        xpack_out = torch.empty(lib.nvfp4_gemm_packed_act_bytes(M, N // 2), dtype=torch.uint8, device=xpack.device)
+    if workspace is None:
+        workspace = nvfp4_gemm_packed_new_workspace(M, N, K, xpack.device)
+    _check(lib.nvfp4_gemm_packed_silu_quant_out(_ptr(w_blob_gate_up), _ptr(w_gscale), N, K, _ptr(xpack), _ptr(x_gscale),
+                                                1 if gscale_per_row else 0, M, _ptr(h), h_dtype, h.stride(0) if h is not None else N // 2,
+                                                _ptr(xpack_out), _ptr(out_gscale), _ptr(workspace), workspace.numel(), _stream()))
+    return xpack_out, h
 
 
 NOALLOC_SCRATCH_BYTES = 4 << 20

@@ -433,4 +433,43 @@ int nvfp4_gemm_w4a16(const void* w_blob_tc, const float* w_gscale, int N, int K,
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+// ---- fused gate_up: interleaved blob + SiLU * mul + static-scale quantizer in the GEMM epilogue ----
+static bool gate_up_shape_ok(int N, int K) { return N >= 128 && (N % 128) == 0 && gemm_tc_supported(N, K); }
+
+int nvfp4_gemm_repack_weight_gate_up(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!codes || !scales || !blob_out) return NVFP4_ERR_INVALID_ARG;
+    if (N < 1 || K < 1 || !gate_up_shape_ok(N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(codes) || !aligned16(scales) || !aligned16(blob_out)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_repack_tc(codes, scales, N, K, blob_out, static_cast<cudaStream_t>(stream), 1);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemm_unpack_weight_gate_up(const void* blob, int N, int K, uint8_t* codes_out, uint8_t* scales_out, void* stream) {
+    g_last_err[0] = 0;
+    if (!codes_out || !scales_out || !blob) return NVFP4_ERR_INVALID_ARG;
+    if (N < 1 || K < 1 || !gate_up_shape_ok(N, K)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(codes_out) || !aligned16(scales_out) || !aligned16(blob)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_unpack_tc(blob, N, K, codes_out, scales_out, static_cast<cudaStream_t>(stream), 1);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemm_packed_silu_quant_out(const void* w_blob_gate_up, const float* w_gscale, int N, int K, const void* xpack,
+                                     const float* x_gscale, int gscale_per_row, int M, void* h_opt, int h_dtype, int64_t ldh,
+                                     void* xpack_out, const float* out_gscale, void* workspace, size_t ws_bytes, void* stream) {
+    g_last_err[0] = 0;
+    if (h_dtype != NVFP4_DTYPE_F32 && h_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_per_row != 0 && gscale_per_row != 1) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob_gate_up || !w_gscale || !xpack || !x_gscale || !xpack_out || !out_gscale || !workspace) return NVFP4_ERR_INVALID_ARG;
+    if (M < 1 || M > 128 || N < 1 || K < 1 || !gate_up_shape_ok(N, K) || ((N / 2) % 256) != 0 || (h_opt && ldh < N / 2))
+        return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob_gate_up) || !aligned16(xpack) || (h_opt && !aligned16(h_opt)) || !aligned16(xpack_out) || !aligned16(workspace) ||
+        (reinterpret_cast<uintptr_t>(w_gscale) & 3u) || (reinterpret_cast<uintptr_t>(x_gscale) & 3u) ||
+        (reinterpret_cast<uintptr_t>(out_gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    if (ws_bytes < gemm_tc_packed_workspace_bytes(M, N, K)) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemm_tc_packed(w_blob_gate_up, w_gscale, N, K, xpack, x_gscale, gscale_per_row, M, h_opt, h_dtype, ldh,
+                                          workspace, ws_bytes, static_cast<cudaStream_t>(stream), xpack_out, out_gscale, N / 2, 1);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 }  // extern "C"

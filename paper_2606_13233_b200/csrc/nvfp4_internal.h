@@ -84,9 +84,9 @@ cudaError_t launch_pack_x(const uint8_t* x_codes, int64_t ldx, const uint8_t* x_
 cudaError_t launch_gemm_tc_packed(const void* blob, const float* w_gscale, int N, int K, const void* xpack,
                                   const float* x_gscale, int gscale_per_row, int M, void* y, int y_dtype, int64_t ldy,
                                   void* workspace, size_t ws_bytes, cudaStream_t st, void* qout = nullptr,
-                                  const float* qout_gscale = nullptr, int n_quant = 0);
-cudaError_t launch_repack_tc(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob, cudaStream_t st);
-cudaError_t launch_unpack_tc(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st);
+                                  const float* qout_gscale = nullptr, int n_quant = 0, int silu = 0);
+cudaError_t launch_repack_tc(const uint8_t* codes, const uint8_t* scales, int N, int K, void* blob, cudaStream_t st, int inter = 0);
+cudaError_t launch_unpack_tc(const void* blob, int N, int K, uint8_t* codes, uint8_t* scales, cudaStream_t st, int inter = 0);
 cudaError_t launch_gemm_tc(const void* blob, const float* w_gscale, int N, int K, const uint8_t* x_codes, int64_t ldx,
                            const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, void* y, int y_dtype,
                            int64_t ldy, void* workspace, size_t ws_bytes, cudaStream_t st);

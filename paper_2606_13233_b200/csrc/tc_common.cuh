@@ -14,8 +14,15 @@ constexpr uint32_t TC_BLOB_MAGIC = 0x5446564Eu;         // "NVFT"
 
 __host__ __device__ inline int tc_tiles(int N) { return (N + TC_TILE_N - 1) / TC_TILE_N; }
 __host__ __device__ inline int tc_xrec_bytes(int MT) { return MT * 128 + TC_SF_BYTES; }
-__host__ __device__ inline uint4 tc_header_words(int N, int K) {
-    return make_uint4(TC_BLOB_MAGIC, ((uint32_t)NVFP4_ABI_VERSION << 16) | 0x7Cu, (uint32_t)N, (uint32_t)K);
+// `interleaved` (fused gate_up weights, N = 2I): tile t holds gate rows [64t, 64t+64) in its rows 0..63 and the matching up
+// rows [I + 64t, I + 64t + 64) in its rows 64..127, so that one tile's epilogue owns both factors of SiLU(gate) * up
+__host__ __device__ inline uint4 tc_header_words(int N, int K, int interleaved = 0) {
+    return make_uint4(TC_BLOB_MAGIC, ((uint32_t)NVFP4_ABI_VERSION << 16) | (interleaved ? 0x7Du : 0x7Cu), (uint32_t)N, (uint32_t)K);
+}
+// canonical weight row held by row r of tile `tile`
+__host__ __device__ inline int tc_source_row(int tile, int r, int N, int interleaved) {
+    if (!interleaved) return tile * TC_TILE_N + r;
+    return r < 64 ? tile * 64 + r : N / 2 + tile * 64 + (r - 64);
 }
 
 // ---- tcgen05 / TMEM wrappers (PTX ISA "tcgen05" family; B200 guide sec. 1-2) ---------------------------------------

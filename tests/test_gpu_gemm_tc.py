@@ -249,3 +249,62 @@ def test_fused_output_quantizer_feeds_next_gemm(B):
     oc, os_, og = orc.quantize(y1f, g=np.float32(0.004))
     Y2, A2 = orc.gemv_w4a4(w2c, w2s, g2, oc, os_, og)
     U.check_gemv(U.host_y_f64(y2), Y2, A2, "GEMM2 on records written by GEMM1's epilogue")
+
+
+def test_gate_up_interleaved_repack_round_trip(B):
+    rng = np.random.default_rng(5)
+    for N, K in [(128, 256), (1024, 512), (1536, 256)]:
+        wc = rng.integers(0, 256, (N, K // 2), dtype=np.uint8)
+        ws = rng.integers(0, 0x7F, (N, K // 16), dtype=np.uint8)
+        blob = B.nvfp4_gemm_repack_weight_gate_up(U.dev_u8(wc), U.dev_u8(ws))
+        c2, s2 = B.nvfp4_gemm_unpack_weight_gate_up(blob, N, K)
+        assert np.array_equal(U.host_u8(c2), wc) and np.array_equal(U.host_u8(s2), ws)
+        # tile 0 of the interleaved blob = gate rows 0..63 then up rows I..I+63: its first code chunk rows
+        plain = U.host_u8(B.nvfp4_gemm_repack_weight(U.dev_u8(np.concatenate([wc[:64], wc[N // 2:N // 2 + 64]])),
+                                                     U.dev_u8(np.concatenate([ws[:64], ws[N // 2:N // 2 + 64]]))))
+        KS = K // 256
+        assert np.array_equal(U.host_u8(blob)[128:128 + KS * 18432], plain[128:128 + KS * 18432])
+
+
+@pytest.mark.parametrize("M,I,K", [(1, 256, 512), (4, 512, 1024), (8, 1024, 512), (20, 512, 768), (2, 25600, 256), (8, 2560, 5120)])
+def test_fused_gate_up_silu_quantizer(B, M, I, K):
+    """gate_up GEMM + SiLU*mul + STATIC quantizer in ONE launch == plain GEMM (BF16 gate_up) -> nvfp4_silu_mul_quantize_packed
+    (STATIC), byte for byte; h equals nvfp4_silu_mul's; the records feed the down GEMM within the oracle tolerance."""
+    N = 2 * I
+    c = make_case(M, N, K, seed=I + K + M)
+    gw, gx = U.dev_f32(c["gw"] * 4), U.dev_f32(c["gx"])                # scaled up a little: silu sees both of its regimes, |gate| stays < 88
+    blob_plain = B.nvfp4_gemm_repack_weight(U.dev_u8(c["wc"]), U.dev_u8(c["ws"]))
+    blob_gu = B.nvfp4_gemm_repack_weight_gate_up(U.dev_u8(c["wc"]), U.dev_u8(c["ws"]))
+    xp = B.nvfp4_gemm_pack_act(U.dev_u8(c["xc"]), U.dev_u8(c["xs"]))
+    y_gu = B.nvfp4_gemm_packed(blob_plain, gw, N, K, xp, gx, M, y_dtype=B.DTYPE_BF16)
+    h_ref = torch.empty((M, I), dtype=torch.bfloat16, device="cuda")
+    B.nvfp4_silu_mul(y_gu, h_ref)
+    torch.cuda.synchronize()
+    hf = orc.bf16_bits_to_f32(U.host_bf16_bits(h_ref))
+    g_static = U.dev_f32(np.float32(max(float(np.max(np.abs(hf))), 1e-6) / 2688.0 * 0.9))
+    want = torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(M, I), dtype=torch.uint8, device="cuda")
+    if M * I <= 524288:
+        B.nvfp4_silu_mul_quantize_packed(y_gu, xpack=want, gscale=g_static.clone(), gscale_mode=B.GSCALE_STATIC)
+    else:
+        B.nvfp4_quantize_act_packed(h_ref, xpack=want, gscale=g_static.clone(), gscale_mode=B.GSCALE_STATIC)
+    out = torch.zeros_like(want)
+    h = torch.zeros((M, I), dtype=torch.bfloat16, device="cuda")
+    B.nvfp4_gemm_packed_silu_quant_out(blob_gu, gw, N, K, xp, gx, M, g_static, xpack_out=out, h=h)
+    torch.cuda.synchronize()
+    assert torch.equal(h, h_ref)
+    assert torch.equal(out, want)
+    # against the oracle: silu_mul of the BF16 gate_up output (1 BF16 ulp), and the quantisation of h itself exactly
+    want_h = orc.silu_mul(orc.bf16_bits_to_f32(U.host_bf16_bits(y_gu)))
+    assert np.all(np.abs(U.host_y_f64(h) - want_h) <= np.maximum(np.abs(want_h), 2.0 ** -120) * 2.0 ** -7)
+    oc, os_, _ = orc.quantize(hf, g=np.float32(g_static.item()))
+    assert torch.equal(out, B.nvfp4_gemm_pack_act(U.dev_u8(oc), U.dev_u8(os_)))
+    # records only (no h)
+    out2 = torch.zeros_like(want)
+    B.nvfp4_gemm_packed_silu_quant_out(blob_gu, gw, N, K, xp, gx, M, g_static, xpack_out=out2, h=None)
+    torch.cuda.synchronize()
+    assert torch.equal(out2, want)
+    # the wrong blob kind must not produce plausible numbers
+    hh = torch.zeros((M, I), dtype=torch.bfloat16, device="cuda")
+    B.nvfp4_gemm_packed_silu_quant_out(blob_plain, gw, N, K, xp, gx, M, g_static, xpack_out=out2, h=hh)
+    assert torch.isnan(hh).all()
+    assert torch.isnan(B.nvfp4_gemm_packed(blob_gu, gw, N, K, xp, gx, M, y_dtype=B.DTYPE_F32)).all()
