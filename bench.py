@@ -777,9 +777,12 @@ def run_chain(args):
     for M, fused, producer, tc in ((1, False, True, 0), (2, False, True, 0), (4, False, True, 0), (8, False, True, 0),
                                    (1, True, True, 0), (1, False, False, 0), (1, True, False, 0),
                                    (1, False, True, 1), (2, False, True, 1), (4, False, True, 1), (8, False, True, 1), (32, False, True, 1),
-                                   (1, False, True, 2), (2, False, True, 2), (4, False, True, 2), (8, False, True, 2), (32, False, True, 2)):
-        # tc: 0 = CUDA-core GEMV, 1 = tensor-core GEMM with quantizer launches, 2 = tensor-core GEMM, static scales, fused quantizers
-        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer, tensor_core=tc > 0, static_scales=tc == 2)
+                                   (1, False, True, 2), (2, False, True, 2), (4, False, True, 2), (8, False, True, 2), (16, False, True, 2), (32, False, True, 2),
+                                   (1, False, True, 3), (2, False, True, 3), (4, False, True, 3), (8, False, True, 3), (16, False, True, 3), (32, False, True, 3)):
+        # tc: 0 = CUDA-core GEMV, 1 = tensor-core GEMM with quantizer launches, 2 = tensor-core GEMM, static scales, quantizers fused
+        # into the GEMM epilogues (gate_up: own launch for SiLU*mul+quantize), 3 = 2 with SiLU*mul+quantize in gate_up's epilogue too
+        ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer, tensor_core=tc > 0, static_scales=tc >= 2,
+                         fuse_gate_up=tc == 3)
         h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
         ch.calibrate(h0)
         ch.step()

@@ -211,7 +211,8 @@ int nvfp4_get_layout_kparts(int N, int K);
  * as nvfp4_silu_mul), then the NVFP4 quantizer of nvfp4_quantize_act on h[M,I].  codes / scales / gscale are
  * bit-identical to nvfp4_silu_mul followed by nvfp4_quantize_act; the BF16 intermediate is not written unless
  * h_bf16_opt is given.
- *   gu_bf16 [device] BF16 [M, 2I], row stride 2I;  I % 16 == 0, M*I <= 524288
+ *   gu_bf16 [device] BF16 [M, 2I], row stride 2I;  I % 16 == 0;  M*I <= 524288 unless gscale_mode is NVFP4_GSCALE_STATIC
+ *           (a given scale needs no tensor-wide amax: plain wide grid instead of one thread-block cluster, any size)
  *   codes [device] out uint8 [M, I/2];  scales [device] out uint8 [M, I/16];  gscale as for nvfp4_quantize_act
  *   h_bf16_opt [device] optional (may be NULL): BF16 [M, I] copy of the intermediate
  */
@@ -292,7 +293,7 @@ int nvfp4_gemm(const void* w_blob_tc, const float* w_gscale, int N, int K,
  *   nvfp4_quantize_act_packed       nvfp4_quantize_act writing the packed layout directly: the same binary32 sequence,
  *                                   so pack_act(quantize_act(x)) == quantize_act_packed(x) byte for byte.  M <= 128 for
  *                                   NVFP4_GSCALE_DYNAMIC / _STATIC, M <= 8 for _DYNAMIC_PER_ROW.
- *   nvfp4_silu_mul_quantize_packed  nvfp4_silu_mul_quantize writing the packed layout (M * I <= 524288)
+ *   nvfp4_silu_mul_quantize_packed  nvfp4_silu_mul_quantize writing the packed layout (M * I <= 524288 unless _STATIC)
  *   nvfp4_gemm_packed               the GEMM on packed activations; workspace >= nvfp4_gemm_packed_workspace_bytes,
  *                                   zero-filled once; other arguments as for nvfp4_gemm
  *   nvfp4_gemm_set_config           tuning knobs (0 = table), process-wide like nvfp4_gemv_set_config: depth of the

@@ -20,11 +20,17 @@ QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
 
 class DecodeChain:
     def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False,
-                 fused_producer: bool = True, tensor_core: bool = False, static_scales: bool = False):
+                 fused_producer: bool = True, tensor_core: bool = False, static_scales: bool = False,
+                 fuse_gate_up: bool = False):
         # static_scales (tensor-core path only; the paper's deployed flow): every projection's input global
         # scale is fixed by calibrate(), and each GEMM quantises the NEXT projection's input in its own epilogue
         # (nvfp4_gemm_packed_quant_out): 5 launches per layer -- 4 GEMMs + the SiLU*mul/quantize producer
         self.static_scales = static_scales and tensor_core
+        # fuse_gate_up: SiLU*mul + quantize in gate_up's own epilogue (nvfp4_gemm_packed_silu_quant_out, 4 launches per layer).
+        # Off by default: measured slower in the chain at every M (profiles/r02_sweep.md) -- the separate producer launch
+        # hides under the down GEMM's pipeline fill, while the fused epilogue lengthens gate_up's tail (and for M > 16 its
+        # 8-row passes on two of the four epilogue warps outlast a tile's streaming time).
+        self.fuse_gate_up = self.static_scales and bool(fuse_gate_up)
         self.tensor_core = tensor_core                # projections on the tcgen05 GEMM (nvfp4_quantize_act_packed +
                                                       # nvfp4_gemm_packed, M <= 128) instead of the CUDA-core GEMV
         if tensor_core:
@@ -38,6 +44,8 @@ class DecodeChain:
         self.shapes = (("qkv", QKV, H), ("o", H, OIN), ("gate_up", 2 * I, H), ("down", H, I))
         self.w = []                                   # per layer: list of (blob, gW tensor, N, K)
         self.canon = []                               # canonical bytes kept only when asked (tests)
+        gu_blobs = []                                 # static chain: gate_up again, rows interleaved per tile (fused SiLU*mul epilogue)
+        self.gu_blobs = gu_blobs
         for l in range(layers):
             row = []
             for sid, (name, N, K) in enumerate(self.shapes):
@@ -46,6 +54,8 @@ class DecodeChain:
                 g = 1.0 / (557.0 * math.sqrt(K))       # keeps activations O(1) through the chain
                 blob = B.nvfp4_gemm_repack_weight(codes, scales) if tensor_core else B.nvfp4_repack_weight(codes, scales)
                 row.append((blob, torch.tensor([g], dtype=torch.float32, device=device), N, K))
+                if self.fuse_gate_up and name == "gate_up":
+                    gu_blobs.append(B.nvfp4_gemm_repack_weight_gate_up(codes, scales))
                 del codes, scales
             self.w.append(row)
         bf, u8 = torch.bfloat16, torch.uint8
@@ -67,7 +77,7 @@ class DecodeChain:
             self.ws = [B.new_workspace(M, N, K, device) for _, N, K in self.shapes]
         self.launches_per_step = layers * ((5 if fused else 8) if fused_producer else (5 if fused else 9))
         if self.static_scales:
-            self.launches_per_step = 1 + (5 if M * I <= 524288 else 6) * layers
+            self.launches_per_step = 1 + (4 if self.fuse_gate_up else 5) * layers
 
     def set_input(self, h_bf16):
         self.h.copy_(h_bf16)
@@ -104,7 +114,8 @@ class DecodeChain:
 
     def _step_static(self, taps=None):
         """tensor-core chain with static activation scales: one quantizer launch for the token's input, then per layer
-        QKV(+quant for O) -> O(+quant for gate_up) -> gate_up -> SiLU*mul+quantize -> down(+quant for the next QKV)."""
+        QKV(+quant for O) -> O(+quant for gate_up) -> gate_up -> SiLU*mul+quantize -> down(+quant for the next QKV)
+        (fuse_gate_up: gate_up(+SiLU*mul+quant for down) in one launch)."""
         d, M, S = self.d, self.M, B.GSCALE_STATIC
         H, OIN, I = d["hidden"], d["o_in"], d["inter"]
         keep = taps is not None
@@ -117,12 +128,13 @@ class DecodeChain:
                                           y=self.y_qkv if keep else None, workspace=self.ws[0])
             B.nvfp4_gemm_packed_quant_out(bo, go, No, Ko, b, self.gs[l][1], M, self.gs[l][2], n_quant=H, xpack_out=a,
                                           y=self.y_o if keep else None, workspace=self.ws[1])
-            B.nvfp4_gemm_packed(bg, gg, Ng, Kg, a, self.gs[l][2], M, y=self.y_gu, y_dtype=B.DTYPE_BF16, workspace=self.ws[2])
-            if M * I <= 524288:
-                B.nvfp4_silu_mul_quantize_packed(self.y_gu, b, self.gs[l][3], gscale_mode=S, h_out=self.act if keep else None)
+            if keep or not self.fuse_gate_up:             # (fused form: the plain BF16 gate_up output only for the tests)
+                B.nvfp4_gemm_packed(bg, gg, Ng, Kg, a, self.gs[l][2], M, y=self.y_gu, y_dtype=B.DTYPE_BF16, workspace=self.ws[2])
+            if self.fuse_gate_up:
+                B.nvfp4_gemm_packed_silu_quant_out(self.gu_blobs[l], gg, Ng, Kg, a, self.gs[l][2], M, self.gs[l][3], xpack_out=b,
+                                                   h=self.act if keep else None, workspace=self.ws[2])
             else:
-                B.nvfp4_silu_mul(self.y_gu, self.act)
-                B.nvfp4_quantize_act_packed(self.act, b, self.gs[l][3], gscale_mode=S)
+                B.nvfp4_silu_mul_quantize_packed(self.y_gu, b, self.gs[l][3], gscale_mode=S, h_out=self.act if keep else None)
             if l + 1 < self.layers:
                 B.nvfp4_gemm_packed_quant_out(bd, gd, Nd, Kd, b, self.gs[l][3], M, self.gs[l + 1][0], n_quant=H, xpack_out=a,
                                               y=self.h if keep else None, workspace=self.ws[3])

@@ -259,7 +259,7 @@ int nvfp4_silu_mul_quantize(const void* gu_bf16, int M, int I, uint8_t* codes, u
     if (!gu_bf16 || !codes || !scales || !gscale) return NVFP4_ERR_INVALID_ARG;
     if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC &&
         gscale_mode != NVFP4_GSCALE_DYNAMIC_PER_ROW) return NVFP4_ERR_INVALID_ARG;
-    if (!shape_ok(M, 1, I) || (int64_t)M * I > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!shape_ok(M, 1, I) || (gscale_mode != NVFP4_GSCALE_STATIC && (int64_t)M * I > 524288)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     if (!aligned16(gu_bf16) || !aligned16(codes) || !aligned16(scales) || (h_bf16_opt && !aligned16(h_bf16_opt)) ||
         (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
     cudaError_t e = launch_silu_mul_quantize(gu_bf16, M, I, codes, scales, gscale, gscale_mode, h_bf16_opt,
@@ -363,7 +363,8 @@ int nvfp4_silu_mul_quantize_packed(const void* gu_bf16, int M, int I, void* xpac
     if (!gu_bf16 || !xpack_out || !gscale) return NVFP4_ERR_INVALID_ARG;
     if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC &&
         gscale_mode != NVFP4_GSCALE_DYNAMIC_PER_ROW) return NVFP4_ERR_INVALID_ARG;
-    if (M < 1 || M > 128 || I < 1 || !gemm_tc_supported(1, I) || (int64_t)M * I > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (M < 1 || M > 128 || I < 1 || !gemm_tc_supported(1, I)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (gscale_mode != NVFP4_GSCALE_STATIC && (int64_t)M * I > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;   // one cluster (amax on chip)
     if (gscale_mode == NVFP4_GSCALE_DYNAMIC_PER_ROW && M > 8) return NVFP4_ERR_UNSUPPORTED_SHAPE;
     if (!aligned16(gu_bf16) || !aligned16(xpack_out) || (h_bf16_opt && !aligned16(h_bf16_opt)) ||
         (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;

@@ -155,16 +155,16 @@ def test_chain_tensor_core_full_size_m8():
     assert torch.isfinite(ch.h.float()).all()
 
 
-@pytest.mark.parametrize("M", [1, 8, 24])
-def test_chain_tensor_core_static_scales_fused_quantizers(M):
+@pytest.mark.parametrize("M,fuse", [(1, False), (1, True), (4, True), (8, False), (8, True), (24, False), (24, True)])
+def test_chain_tensor_core_static_scales_fused_quantizers(M, fuse):
     """tensor-core chain with static activation scales: no quantizer launches between projections (each GEMM's epilogue
-    writes the next GEMM's packed NVFP4 input).  Every projection is checked against the oracle: quantize(its BF16 input,
-    static g) -> float64 GEMV on the unpacked weights."""
+    writes the next GEMM's packed NVFP4 input; with `fuse`, gate_up's also applies SiLU * mul: 4 launches per layer).  Every projection
+    is checked against the oracle: quantize(its BF16 input, static g) -> float64 GEMV on the unpacked weights."""
     from paper_2606_13233_b200 import binding as B
     from paper_2606_13233_b200.chain import DecodeChain
     dims = dict(hidden=512, qkv=768, o_in=512, inter=768)
-    ch = DecodeChain(layers=3, M=M, dims=dims, seed=8, tensor_core=True, static_scales=True)
-    assert ch.launches_per_step == 1 + 5 * 3
+    ch = DecodeChain(layers=3, M=M, dims=dims, seed=8, tensor_core=True, static_scales=True, fuse_gate_up=fuse)
+    assert ch.fuse_gate_up == fuse and ch.launches_per_step == 1 + (4 if fuse else 5) * 3
     h0 = U.dev_bf16_from_bits(inputs.make_activation_bits(M, 512, 0, 81))
     ch.calibrate(h0)
     taps = []
@@ -181,6 +181,14 @@ def test_chain_tensor_core_static_scales_fused_quantizers(M):
         oxc, oxs, ogx = orc.quantize(xf, g=g_static)
         Y, A = orc.gemv_w4a4(U.host_u8(wc), U.host_u8(ws), np.float32(gw.item()), oxc, oxs, ogx)
         U.check_gemv(U.host_y_f64(y), Y, A, f"static tc chain layer {l} {name} M={M}", bf16_slack=True)
+        if name == "gate_up" and ch.fuse_gate_up:
+            # the fused kernel reads the SAME weights from the interleaved blob, and its h (the down tap's input, which the
+            # oracle quantizes above) is SiLU(gate) * up of this projection's BF16 output
+            wc2, ws2 = B.nvfp4_gemm_unpack_weight_gate_up(ch.gu_blobs[l], N, K)
+            assert torch.equal(wc2, wc) and torch.equal(ws2, ws)
+            act = torch.empty(M, N // 2, dtype=torch.bfloat16, device="cuda")
+            B.nvfp4_silu_mul(y.contiguous(), act)
+            assert torch.equal(act, taps[4 * l + 3][2])
     # the timed form (no BF16 outputs between projections) ends on the same bits, eagerly and under graph replay
     ref = ch.h.clone()
     ch.set_input(h0); ch.step(); torch.cuda.synchronize()

@@ -194,6 +194,28 @@ def test_silu_mul_quantize_packed(B):
     assert np.array_equal(U.host_u8(got), want) and torch.equal(g, g2)
 
 
+def test_silu_mul_quantize_packed_static_any_size(B):
+    """a STATIC scale needs no tensor-wide amax: plain wide grid, no M * I limit (the DYNAMIC modes keep theirs: one cluster)"""
+    M, I = 32, 25600
+    rng = np.random.default_rng(5)
+    gu = torch.from_numpy((rng.standard_normal((M, 2 * I)) * 2).astype(np.float32)).cuda().to(torch.bfloat16)
+    gs = U.dev_f32(np.float32(0.003))
+    h = torch.empty((M, I), dtype=torch.bfloat16, device="cuda")
+    zeros = lambda m: torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(m, I), dtype=torch.uint8, device="cuda")   # (records have unused bytes)
+    got, _ = B.nvfp4_silu_mul_quantize_packed(gu, xpack=zeros(M), gscale=gs.clone(), gscale_mode=B.GSCALE_STATIC, h_out=h)
+    h2 = B.nvfp4_silu_mul(gu)
+    want, _ = B.nvfp4_quantize_act_packed(h2, xpack=zeros(M), gscale=gs.clone(), gscale_mode=B.GSCALE_STATIC)
+    assert torch.equal(h, h2) and torch.equal(got, want)
+    # rows 8..15 through the canonical quantizer (M <= 8 there) and the oracle
+    xc, xs, _ = B.nvfp4_quantize_act(h2[8:16].contiguous(), gscale=gs.clone(), gscale_mode=B.GSCALE_STATIC)
+    oc, os_, _ = orc.quantize(orc.bf16_bits_to_f32(U.host_bf16_bits(h2[8:16].contiguous())), g=np.float32(0.003))
+    assert np.array_equal(U.host_u8(xc), oc) and np.array_equal(U.host_u8(xs), os_)
+    sub, _ = B.nvfp4_quantize_act_packed(h2[8:16].contiguous(), xpack=zeros(8), gscale=gs.clone(), gscale_mode=B.GSCALE_STATIC)
+    assert torch.equal(sub, B.nvfp4_gemm_pack_act(xc, xs, xpack=zeros(8)))
+    with pytest.raises(B.Nvfp4Error):
+        B.nvfp4_silu_mul_quantize_packed(gu)              # DYNAMIC: M * I > 524288
+
+
 @pytest.mark.parametrize("M,N,K,nq", [(1, 512, 512, 512), (8, 1024, 2048, 768), (5, 5120, 1024, 5120), (24, 768, 512, 256),
                                        (100, 512, 768, 512), (4, 10240, 5120, 8192), (8, 5120, 8192, 5120)])
 def test_fused_output_quantizer_equals_separate_quantizer_and_oracle(B, M, N, K, nq):
@@ -283,10 +305,7 @@ def test_fused_gate_up_silu_quantizer(B, M, I, K):
     hf = orc.bf16_bits_to_f32(U.host_bf16_bits(h_ref))
     g_static = U.dev_f32(np.float32(max(float(np.max(np.abs(hf))), 1e-6) / 2688.0 * 0.9))
     want = torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(M, I), dtype=torch.uint8, device="cuda")
-    if M * I <= 524288:
-        B.nvfp4_silu_mul_quantize_packed(y_gu, xpack=want, gscale=g_static.clone(), gscale_mode=B.GSCALE_STATIC)
-    else:
-        B.nvfp4_quantize_act_packed(h_ref, xpack=want, gscale=g_static.clone(), gscale_mode=B.GSCALE_STATIC)
+    B.nvfp4_silu_mul_quantize_packed(y_gu, xpack=want, gscale=g_static.clone(), gscale_mode=B.GSCALE_STATIC)
     out = torch.zeros_like(want)
     h = torch.zeros((M, I), dtype=torch.bfloat16, device="cuda")
     B.nvfp4_gemm_packed_silu_quant_out(blob_gu, gw, N, K, xp, gx, M, g_static, xpack_out=out, h=h)
