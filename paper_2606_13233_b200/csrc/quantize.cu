@@ -48,6 +48,12 @@ struct LoadX {
         const uint4* p = reinterpret_cast<const uint4*>(x + (int64_t)m * ldx + (int64_t)kb * 16);
         a = __ldg(p); b = __ldg(p + 1);
     }
+    // L2 prefetch of the block's line, issued BEFORE griddepcontrol.wait: harmless whoever writes X (L2 is the point of
+    // coherence), and when X is not the predecessor's output (a fresh token's hidden state, DRAM-cold) the loads after the
+    // wait find it in L2
+    __device__ __forceinline__ void prefetch(int m, int kb) const {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(x + (int64_t)m * ldx + (int64_t)kb * 16));
+    }
 };
 // fused SiLU*mul (step a8 + a1 + a2 in one launch): the block is
 // h[m, 16kb..] = RN_bf16(silu(gu[m, j]) * gu[m, I + j]) -- the same FP32 expression and BF16 rounding as
@@ -75,6 +81,7 @@ struct LoadSiluMul {
             ph[0] = a; ph[1] = b;
         }
     }
+    __device__ __forceinline__ void prefetch(int, int) const {}      // (gate_up was just written: L2-hot)
 };
 
 constexpr int QMODE_STATIC = 0, QMODE_DYNAMIC = 1, QMODE_DYNAMIC_PER_ROW = 2;
@@ -111,6 +118,11 @@ quantize_act_kernel(Loader load, int M, int K, uint8_t* __restrict__ codes, uint
     // right before the DSMEM stores (the latency hides under the loads)
     if (QMODE != QMODE_STATIC && gridDim.x > 1) asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
     if (QMODE == QMODE_DYNAMIC_PER_ROW && threadIdx.x < 8) row_max[threadIdx.x] = 0u;
+#pragma unroll
+    for (int i = 0; i < BPT; ++i) {
+        const int b = gtid + i * nthreads;
+        if (b < NB) load.prefetch(b / kb_per_row, b % kb_per_row);
+    }
     pdl_wait();                                       // X is the previous kernel's output
     pdl_launch_dependents();                          // the GEMV may start streaming its weights now
 
