@@ -14,6 +14,10 @@
  *     unless it returns a size or a string.
  *   - Every pointer marked [device] is CUDA device memory owned by the CALLER and must be
  *     16-byte aligned; the library never allocates, frees or retains caller memory.
+ *     Pinned, device-mapped HOST memory (cudaHostAlloc / cudaHostRegister under unified addressing) qualifies
+ *     for the BF16 activation inputs and the y outputs: the kernels then read / write it over PCIe themselves
+ *     ("zero-copy"; each activation element is read once, each output written once).  Weights, workspaces and
+ *     the NVFP4 intermediates belong in device memory.
  *   - Calls are ASYNCHRONOUS: they enqueue kernels on `stream` (a cudaStream_t passed as
  *     void*, NULL = the legacy default stream) and return; they never synchronise, never
  *     read device data on the host, and are capturable in a CUDA graph.

@@ -204,3 +204,40 @@ def test_linear_any_m(B, M):
     # chunks reproduce the 8-row GEMV exactly
     y8 = B.nvfp4_gemv(B.MODE_W4A4, blob, U.dev_f32(gw), N, K, U.dev_u8(oxc[:8]), U.dev_u8(oxs[:8]), U.dev_f32(ogx), y_dtype=B.DTYPE_F32)
     assert torch.equal(y[:8], y8)
+
+
+# ---- pinned, device-mapped host buffers (zero-copy; bench.py's e2e form) -----------------------------------------
+@pytest.mark.parametrize("M", [1, 5])
+def test_pinned_host_activations_and_outputs(B, M):
+    """BF16 activations read from, and BF16 outputs written to, pinned HOST memory by the kernels themselves: same bits
+    as with device buffers (CUDA-core GEMV and tensor-core GEMM paths)."""
+    N, K = 1024 + 32, 2048
+    wc, ws, gw = U.oracle_weight(N, K, 5, M)
+    d_gw = U.dev_f32(gw)
+    xbits = inputs.make_activation_bits(M, K, 5, M)
+    x_dev = U.dev_bf16_from_bits(xbits)
+    x_pin = torch.from_numpy(xbits.view(np.int16)).view(torch.bfloat16).pin_memory()
+    # CUDA-core path
+    blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws))
+    c1, s1, g1 = B.nvfp4_quantize_act(x_dev)
+    c2, s2, g2 = torch.empty_like(c1), torch.empty_like(s1), torch.zeros_like(g1)
+    B.nvfp4_quantize_act(x_pin, c2, s2, g2)
+    y_dev = B.nvfp4_gemv(B.MODE_W4A4, blob, d_gw, N, K, c1, s1, g1, y_dtype=B.DTYPE_BF16)
+    y_pin = torch.zeros((M, N), dtype=torch.bfloat16).pin_memory()
+    B.nvfp4_gemv(B.MODE_W4A4, blob, d_gw, N, K, c2, s2, g2, y=y_pin, y_dtype=B.DTYPE_BF16, workspace=B.new_workspace(M, N, K, "cuda"))
+    torch.cuda.synchronize()
+    assert torch.equal(c1, c2) and torch.equal(s1, s2) and torch.equal(g1, g2)
+    assert torch.equal(y_dev.cpu(), y_pin)
+    # tensor-core path (N a multiple of 128 there)
+    Nt = 1024
+    blob_tc = B.nvfp4_gemm_repack_weight(U.dev_u8(wc[:Nt]), U.dev_u8(ws[:Nt]))
+    xp1, gx1 = B.nvfp4_quantize_act_packed(x_dev, xpack=torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device="cuda"))
+    xp2, gx2 = B.nvfp4_quantize_act_packed(x_pin, xpack=torch.zeros(B.lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device="cuda"),
+                                           gscale=torch.zeros(1, dtype=torch.float32, device="cuda"))
+    yt_dev = B.nvfp4_gemm_packed(blob_tc, d_gw, Nt, K, xp1, gx1, M, y_dtype=B.DTYPE_BF16)
+    yt_pin = torch.zeros((M, Nt), dtype=torch.bfloat16).pin_memory()
+    B.nvfp4_gemm_packed(blob_tc, d_gw, Nt, K, xp2, gx2, M, y=yt_pin, y_dtype=B.DTYPE_BF16,
+                        workspace=B.nvfp4_gemm_packed_new_workspace(M, Nt, K, "cuda"))
+    torch.cuda.synchronize()
+    assert torch.equal(xp1, xp2) and torch.equal(gx1, gx2)
+    assert torch.equal(yt_dev.cpu(), yt_pin)
