@@ -111,10 +111,14 @@ class Workload:
     """device state of the step: `copies` distinct weight sets, per-projection activation,
     NVFP4 activation, output and workspace buffers."""
 
-    def __init__(self, M, copies=2, mode="w4a4", shapes=SHAPES):
+    def __init__(self, M, copies=2, mode="w4a4", shapes=SHAPES, records=None):
         import torch
         from paper_2606_13233_b200 import binding as B
         self.torch, self.B, self.M, self.mode, self.shapes = torch, B, M, mode, shapes
+        # M = 1, W4A4 on CUDA cores: quantizer -> GEMV through the GEMV's own activation records (nvfp4_quantize_act_records +
+        # nvfp4_gemv_records: same arithmetic and bits as nvfp4_quantize_act + nvfp4_gemv, one bulk copy instead of the GEMV's
+        # load / decode / store staging).  records=False: the canonical pair.
+        self.records = (mode == "w4a4" and M == 1) if records is None else bool(records)
         self.proj = []
         for sid, (name, N, K) in enumerate(shapes, start=1):
             blobs = []
@@ -133,6 +137,7 @@ class Workload:
                 gx=torch.zeros(1, dtype=torch.float32, device="cuda"),
                 y=torch.empty((M, N), dtype=torch.bfloat16, device="cuda"),
                 xp=(torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, K), dtype=torch.uint8, device="cuda") if mode == "tc" else None),
+                xrec=(B.nvfp4_new_xrecords(N, K, "cuda") if self.records else None),
                 ws=(B.nvfp4_gemm_packed_new_workspace(M, N, K, "cuda") if mode == "tc" else
                     torch.zeros(B.lib.nvfp4_gemm_w4a16_workspace_bytes(M, N, K), dtype=torch.uint8, device="cuda") if mode == "w4a16tc"
                     else B.new_workspace(M, N, K))))
@@ -166,6 +171,8 @@ class Workload:
     def quantize(self, p):
         if self.mode == "tc":
             self.B.nvfp4_quantize_act_packed(p["x"], p["xp"], p["gx"])
+        elif self.records:
+            self.B.nvfp4_quantize_act_records(p["x"], p["xrec"], p["gx"])
         else:
             self.B.nvfp4_quantize_act(p["x"], p["xc"], p["xs"], p["gx"])
 
@@ -176,6 +183,9 @@ class Workload:
                                 y_dtype=B.DTYPE_BF16, workspace=p["ws"])
         elif self.mode == "w4a16tc":   # W4A16 on the tensor cores (activation re-layout + GEMM)
             B.nvfp4_gemm_w4a16(p["blobs"][copy], p["gw"], p["N"], p["K"], p["x"], y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
+        elif self.mode == "w4a4" and self.records:
+            B.nvfp4_gemv_records(p["blobs"][copy], p["gw"], p["N"], p["K"], p["xrec"], p["gx"], y=p["y"], y_dtype=B.DTYPE_BF16,
+                                 workspace=p["ws"])
         elif self.mode == "w4a4":
             B.nvfp4_gemv(B.MODE_W4A4, p["blobs"][copy], p["gw"], p["N"], p["K"], p["xc"], p["xs"], p["gx"],
                          y=p["y"], y_dtype=B.DTYPE_BF16, workspace=p["ws"])
@@ -541,6 +551,17 @@ def run_ours(args):
         ms_step, ms_gemv, ms_q, ms_fused, n_step = time_step_graphs(wl)
     barrier()
     ms_step = max_over_ranks(ms_step, world, "cuda")
+    canonical = None
+    if wl.records and rank == 0:       # the same step through the canonical pair (nvfp4_quantize_act + nvfp4_gemv), for reference
+        wc_ = Workload(M, copies=2, records=False)
+        g_c, _ = wc_.capture(2)
+        g_cg, _ = wc_.capture(2, quant=False)
+        t_c, t_cg = time_graph(torch, g_c, reps, wrep) / 2, time_graph(torch, g_cg, reps, wrep) / 2
+        same = all(bool(torch.equal(a["y"], b["y"])) for a, b in zip(wl.proj, wc_.proj))
+        canonical = {"what": "same step with nvfp4_quantize_act + nvfp4_gemv (canonical codes / scales between the two)",
+                     "ms_per_step": t_c, "gemv_only_ms": t_cg, "outputs_equal": same}
+        del wc_, g_c, g_cg
+        torch.cuda.empty_cache()
 
     # end to end through the public API from pinned HOST buffers, all transfers inside the timed region.  Three forms:
     # copy form as plain stream launches from Python (H2D of the BF16 activations, quantize_act, gemv, D2H of the BF16
@@ -702,7 +723,11 @@ def run_ours(args):
             "config": {"workload": WORKLOAD, "M": M, "l2": "cold: inputs larger than L2 (274 MB weights per step, "
                        "2 distinct weight sets alternate; L2 = 126 MB); per-shape numbers walk >= 4 x L2 of distinct copies",
                        "timing": f"CUDA graph replay, CUDA events, {reps} timed replays of 2 steps (>= {MIN_REPLAYS} whatever --steps)",
+                       "calls": ("nvfp4_quantize_act_records + nvfp4_gemv_records per projection (the GEMV's own activation records "
+                                 "between the two; bit-identical to the canonical pair, see canonical_step)" if canonical is not None or M == 1
+                                 else "nvfp4_quantize_act + nvfp4_gemv per projection"),
                        "multi_gpu": "replicas only"},
+            "canonical_step": canonical,
             "us_per_projection": {"step_mean": round(ms_step * 1e3 / 4, 2), "gemv_mean": round(ms_gemv * 1e3 / 4, 2),
                                   "quantize_mean": round(ms_q * 1e3 / 4, 2),
                                   "per_shape_gemv": per_m.get(str(M), {}).get("per_shape_gemv")},
@@ -712,7 +737,7 @@ def run_ours(args):
             "chain": chain,
             "sampler": sampler,
             "tensor_core": tensor_core,
-            "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone)",
+            "roofline": {"bound": "hbm", "kernel": "gemv_kernel<W4A4> (4 launches per step, timed alone" + (", fed by activation records)" if M == 1 else ")"),
                          "achieved": ach, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": ach / peak,
                          "traffic": TRAFFIC_BYTES_PER_STEP.get(M),
                          "traffic_source": TRAFFIC_SOURCE if M in TRAFFIC_BYTES_PER_STEP else None},

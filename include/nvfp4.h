@@ -210,6 +210,27 @@ int nvfp4_set_layout_kparts(int kparts);
 int nvfp4_get_layout_kparts(int N, int K);
 
 /*
+ * Quantizer -> GEMV through the GEMV's own activation records (M = 1; the decode step, BASELINE.json configs[1]).
+ * nvfp4_gemv stages its activations by loading codes and scales, expanding them and storing them to shared memory after
+ * it has waited for the quantizer; here the quantizer writes that shared-memory image itself (per 32 k: the 2 x 16 E2M1
+ * values as FP16 -- exact --, then the two block scales as FP32; 80 bytes) and the GEMV fetches its K range with ONE
+ * bulk copy.  Same arithmetic, same bits: y equals nvfp4_gemv(NVFP4_MODE_W4A4) on nvfp4_quantize_act's output.
+ *   nvfp4_gemv_xrecord_bytes(N, K)  size of the record buffer for a weight of this shape (K padded to the repacked
+ *                                   layout's cell; depends on the layout's K parts, so query it per weight shape).  The
+ *                                   buffer must be ZERO-FILLED once: the quantizer writes the blocks below K only.
+ *   nvfp4_quantize_act_records      x_bf16 [device] BF16 [1, K]; xrec_out [device] the records; gscale / gscale_mode as for
+ *                                   nvfp4_quantize_act (NVFP4_GSCALE_DYNAMIC or _STATIC); M must be 1
+ *   nvfp4_gemv_records              w_blob / w_gscale / y / workspace as for nvfp4_gemv (same workspace size); xrec from
+ *                                   nvfp4_quantize_act_records for the same K; x_gscale [device] one float; M must be 1
+ * Errors as for nvfp4_gemv; M != 1 -> NVFP4_ERR_UNSUPPORTED_SHAPE.
+ */
+size_t nvfp4_gemv_xrecord_bytes(int N, int K);
+int nvfp4_quantize_act_records(const void* x_bf16, int M, int K, int64_t ldx, void* xrec_out, float* gscale, int gscale_mode,
+                               void* stream);
+int nvfp4_gemv_records(const void* w_blob, const float* w_gscale, int N, int K, const void* xrec, const float* x_gscale, int M,
+                       void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream);
+
+/*
  * SiLU*mul + activation quantizer in ONE launch (the producer of down_proj's input in
  * BASELINE.json configs[4]):  h[m,j] = RN_bf16(silu(gu[m,j]) * gu[m,I+j])  (same FP32 expression and BF16 rounding
  * as nvfp4_silu_mul), then the NVFP4 quantizer of nvfp4_quantize_act on h[M,I].  codes / scales / gscale are

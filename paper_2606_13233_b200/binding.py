@@ -32,7 +32,8 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_quantize_act_packed", "nvfp4_silu_mul_quantize_packed", "nvfp4_gemm_packed_workspace_bytes",
            "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc", "nvfp4_gemm_packed_quant_out",
            "nvfp4_gemm_w4a16", "nvfp4_gemm_w4a16_workspace_bytes", "nvfp4_gemm_repack_weight_gate_up",
-           "nvfp4_gemm_unpack_weight_gate_up", "nvfp4_gemm_packed_silu_quant_out")
+           "nvfp4_gemm_unpack_weight_gate_up", "nvfp4_gemm_packed_silu_quant_out", "nvfp4_gemv_xrecord_bytes",
+           "nvfp4_quantize_act_records", "nvfp4_gemv_records")
 
 
 class Nvfp4Error(RuntimeError):
@@ -74,6 +75,12 @@ def _load():
     lib.nvfp4_set_layout_kparts.argtypes = [c_int]
     lib.nvfp4_get_layout_kparts.restype = c_int
     lib.nvfp4_get_layout_kparts.argtypes = [c_int, c_int]
+    lib.nvfp4_gemv_xrecord_bytes.restype = c_sz
+    lib.nvfp4_gemv_xrecord_bytes.argtypes = [c_int, c_int]
+    lib.nvfp4_quantize_act_records.restype = c_int
+    lib.nvfp4_quantize_act_records.argtypes = [vp, c_int, c_int, c_i64, vp, vp, c_int, vp]
+    lib.nvfp4_gemv_records.restype = c_int
+    lib.nvfp4_gemv_records.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_fused_quant.restype = c_int
     lib.nvfp4_gemv_fused_quant.argtypes = [vp, vp, c_int, c_int, vp, c_int, c_i64, vp, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_set_config.restype = c_int
@@ -403,6 +410,31 @@ def nvfp4_gemv_fused_quant(w_blob, w_gscale, N, K, x_bf16, x_gscale_out=None, y=
     _check(lib.nvfp4_gemv_fused_quant(_ptr(w_blob), _ptr(w_gscale), N, K, _ptr(x_bf16), M, x_bf16.stride(0),
                                       _ptr(x_gscale_out), _ptr(y), y_dtype, y.stride(0), _ptr(workspace),
                                       workspace.numel(), _stream()))
+    return y
+
+
+def nvfp4_new_xrecords(N, K, device):
+    """zero-filled record buffer for nvfp4_quantize_act_records / nvfp4_gemv_records on a weight of shape [N, K]."""
+    return torch.zeros(lib.nvfp4_gemv_xrecord_bytes(N, K), dtype=torch.uint8, device=device)
+
+
+def nvfp4_quantize_act_records(x_bf16, xrec, gscale=None, gscale_mode=GSCALE_DYNAMIC):
+    """BF16 [1,K] -> the CUDA-core GEMV's activation records (xrec from nvfp4_new_xrecords) and g f32 [1]."""
+    M, K = x_bf16.shape
+    if gscale is None:
+        gscale = torch.zeros(1, dtype=torch.float32, device=xrec.device)
+    _check(lib.nvfp4_quantize_act_records(_ptr(x_bf16), M, K, x_bf16.stride(0), _ptr(xrec), _ptr(gscale), gscale_mode, _stream()))
+    return xrec, gscale
+
+
+def nvfp4_gemv_records(w_blob, w_gscale, N, K, xrec, x_gscale, M=1, y=None, y_dtype=DTYPE_BF16, workspace=None):
+    """W4A4 GEMV at M = 1 on activation records (one bulk copy instead of the load / decode / store staging)."""
+    if y is None:
+        y = torch.empty((M, N), dtype=torch.float32 if y_dtype == DTYPE_F32 else torch.bfloat16, device=xrec.device)
+    if workspace is None:
+        workspace = new_workspace(M, N, K, xrec.device)
+    _check(lib.nvfp4_gemv_records(_ptr(w_blob), _ptr(w_gscale), N, K, _ptr(xrec), _ptr(x_gscale), M, _ptr(y), y_dtype,
+                                  y.stride(0), _ptr(workspace), workspace.numel(), _stream()))
     return y
 
 

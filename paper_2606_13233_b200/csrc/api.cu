@@ -357,6 +357,41 @@ int nvfp4_quantize_act_packed(const void* x_bf16, int M, int K, int64_t ldx, voi
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+/* ---- activation records of the CUDA-core GEMV (M = 1): quantizer -> GEMV without the GEMV's load / decode / store stage ---- */
+size_t nvfp4_gemv_xrecord_bytes(int N, int K) {
+    if (!shape_ok(1, N, K)) return 0;
+    const Layout L = make_layout(N, K, effective_kparts(N, K));
+    return (size_t)L.ncells * CELL_VECS * L.kp * GEMV_XRECORD_BYTES;          // one record per 32 k of the padded K
+}
+
+int nvfp4_quantize_act_records(const void* x_bf16, int M, int K, int64_t ldx, void* xrec_out, float* gscale, int gscale_mode,
+                               void* stream) {
+    g_last_err[0] = 0;
+    if (!x_bf16 || !xrec_out || !gscale) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC) return NVFP4_ERR_INVALID_ARG;
+    if (M != 1 || !shape_ok(M, 1, K) || ldx < K || (ldx % 8) != 0) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(x_bf16) || !aligned16(xrec_out) || (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_quantize_act(x_bf16, M, K, ldx, static_cast<uint8_t*>(xrec_out), nullptr, gscale, gscale_mode,
+                                        static_cast<cudaStream_t>(stream), -1);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
+int nvfp4_gemv_records(const void* w_blob, const float* w_gscale, int N, int K, const void* xrec, const float* x_gscale, int M,
+                       void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
+    g_last_err[0] = 0;
+    if (y_dtype != NVFP4_DTYPE_F32 && y_dtype != NVFP4_DTYPE_BF16) return NVFP4_ERR_INVALID_ARG;
+    if (!w_blob || !w_gscale || !xrec || !x_gscale || !y) return NVFP4_ERR_INVALID_ARG;
+    if (M != 1 || !shape_ok(M, N, K) || ldy < N) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(w_blob) || !aligned16(xrec) || !aligned16(y) || (workspace && !aligned16(workspace))) return NVFP4_ERR_ALIGNMENT;
+    const int kp = effective_kparts(N, K);
+    const GemvConfig cfg = effective_config(NVFP4_MODE_W4A4, M, N, K, kp);
+    const size_t need = gemv_workspace_bytes_for(NVFP4_MODE_W4A4, M, N, K, kp, cfg);
+    if (!workspace || ws_bytes < need) return NVFP4_ERR_INVALID_ARG;
+    cudaError_t e = launch_gemv(NVFP4_MODE_W4A4, w_blob, w_gscale, N, K, kp, xrec, nullptr, x_gscale, 0, M, 0, y, y_dtype, ldy,
+                                workspace, ws_bytes, cfg, static_cast<cudaStream_t>(stream), xrec);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 int nvfp4_silu_mul_quantize_packed(const void* gu_bf16, int M, int I, void* xpack_out, float* gscale, int gscale_mode,
                                    void* h_bf16_opt, void* stream) {
     g_last_err[0] = 0;

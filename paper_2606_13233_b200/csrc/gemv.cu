@@ -151,9 +151,11 @@ cudaError_t launch_gemv_w4a4h(const GemvParams& p, int M, int R, dim3 grid, int 
 
 cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, int kp, const void* x,
                         const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, int64_t ldx, void* y,
-                        int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st) {
+                        int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st,
+                        const void* x_records) {
     const bool fuse_quant = (mode == MODE_W4A4_FUSED_QUANT);
     const GemvPlan P = gemv_plan(mode, M, N, K, kp, cfg);
+    if (x_records != nullptr && (mode != NVFP4_MODE_W4A4 || P.kmode != KMODE_W4A4_H)) return cudaErrorInvalidValue;
     if (P.map.total > SMEM_CAP) return cudaErrorInvalidConfiguration;
     if (workspace == nullptr || ws_bytes < counters_bytes(P) + partials_a_bytes(P) + partials_b_bytes(P))
         return cudaErrorInvalidValue;
@@ -188,6 +190,7 @@ cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N
     p.fuse_quant = fuse_quant ? 1 : 0;
     p.gscale_per_row = gscale_per_row;
     p.x_gscale_out = fuse_quant ? const_cast<float*>(x_gscale) : nullptr;
+    p.x_records = static_cast<const uint8_t*>(x_records);
     p.hdr_expect = blob_header_words(N, K, kp);
     p.trace = g_trace;
     dim3 grid(P.nb, P.ksplit);

@@ -67,6 +67,9 @@ struct GemvParams {
     int fuse_quant;                // x is BF16 [M,K] (ldx elements): quantise it inside the kernel (W4A4 modes)
     int gscale_per_row;            // x_gscale holds M per-row (per-token) global scales
     float* x_gscale_out;           // fuse_quant: optional device float that receives the activation global scale
+    const uint8_t* x_records;      // W4A4, M = 1 (FP16 path): activations already in this kernel's shared-memory record layout
+                                   // for the whole padded K (nvfp4_quantize_act_records); each CTA takes its K range with ONE
+                                   // bulk copy instead of loading, decoding and storing it (NULL: x / x_scales are used)
     uint4 hdr_expect;              // blob_header_words(N, K, kp)
     uint32_t smem_map[13];         // gemv_smem_map(...) computed by the host (same order as struct SmemMap)
     unsigned long long* trace;     // debug only (nvfp4_debug_set_trace): 16 timestamps per CTA, else NULL
@@ -92,6 +95,7 @@ __host__ __device__ constexpr int xbp_bytes(int kmode) {
 __host__ __device__ constexpr int xvec_stride(int kmode, int M) {
     return M * xbp_bytes(kmode) + (((M * xbp_bytes(kmode) / 16) % 2 == 0) ? 16 : 0);
 }
+static_assert(xvec_stride(KMODE_W4A4_H, 1) == GEMV_XRECORD_BYTES, "nvfp4_quantize_act_records writes this layout");
 
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     uint32_t d;
@@ -846,7 +850,9 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     uint32_t* red = reinterpret_cast<uint32_t*>(smem + map.misc) + 2;
     c.astart = astart;
     const bool fused = (MODE != KMODE_W4A16) && p.fuse_quant;
-    const int stage_items = fused ? (int)blockDim.x : (int)blockDim.x * STAGE_BATCH;   // items per staging batch
+    const bool records = (MODE == KMODE_W4A4_H) && p.x_records != nullptr;
+    // items per staging batch (records: the one bulk copy covers every item)
+    const int stage_items = records ? (1 << 28) : fused ? (int)blockDim.x : (int)blockDim.x * STAGE_BATCH;
 
     // ---- consumer warps: request the first weight cells before anything else (private ring, private barriers) ----
     // warp w: phase A cells i = w, w + W, ... < na (na_w of them), then phase B cells [bs, be) of the CTA's Bc
@@ -926,6 +932,11 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
     // the weight stream is under way; everything below touches data of the previous kernel
     pdl_wait();
     pdl_launch_dependents();
+    if (MODE == KMODE_W4A4_H && p.x_records != nullptr && threadIdx.x == 0) {   // activation records: first thing after the wait
+        const uint32_t bytes = (uint32_t)(ncw * CELL_VECS * p.kp) * (uint32_t)xvec_stride(MODE, M);
+        mbar_arrive_expect_tx(smem_u32(xbars), bytes);
+        bulk_g2s(smem_u32(xs), p.x_records + (size_t)(c0 * CELL_VECS * p.kp) * xvec_stride(MODE, M), bytes, smem_u32(xbars));
+    }
     NVFP4_CLK(9);
     if (threadIdx.x == 0) NVFP4_TRACE(2);
     // global scales: issue the loads now, combine them only when the first segment is written
@@ -955,7 +966,13 @@ __global__ void __launch_bounds__(gemv_max_threads(MODE, M, R)) gemv_kernel(cons
         }
     };
     // activation staging: every thread of the CTA takes its share
-    if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, deferred);
+    if (records) {
+        // the quantizer wrote the records (32 f16 values + two FP32 block scales per 32 k, padded K zero): one bulk copy of
+        // this CTA's K range, completion on the first staging barrier together with every thread's arrival
+        // (requested right behind griddepcontrol.wait, above)
+        deferred();
+        if (threadIdx.x != 0) mbar_arrive(smem_u32(xbars));
+    } else if (MODE == KMODE_W4A16) stage_x_w4a16<M>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, deferred);
     else if (fused) {
         deferred();
         stage_x_fused<M, MODE == KMODE_W4A4_H>(p, xs, c0, ncw, threadIdx.x, blockDim.x, xbars, red, gx_slot);

@@ -60,7 +60,10 @@ size_t gemv_workspace_bytes_for(int mode, int M, int N, int K, int kp, const Gem
 size_t gemv_smem_bytes(int mode, int M, int N, int K, int kp, const GemvConfig& c);
 cudaError_t launch_gemv(int mode, const void* blob, const float* w_gscale, int N, int K, int kp, const void* x,
                         const uint8_t* x_scales, const float* x_gscale, int gscale_per_row, int M, int64_t ldx, void* y,
-                        int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st);
+                        int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, const GemvConfig& cfg, cudaStream_t st,
+                        const void* x_records = nullptr);
+// activation records of the M = 1 FP16 path (gemv_kernel.cuh XBP_W4A4H): 80 bytes per 32 k = 32 f16 | 2 x FP32 scale | pad
+constexpr int GEMV_XRECORD_BYTES = 80;
 
 cudaError_t launch_silu_mul(const void* gu, int M, int I, void* h, cudaStream_t st);
 

@@ -89,8 +89,19 @@ constexpr int QMODE_STATIC = 0, QMODE_DYNAMIC = 1, QMODE_DYNAMIC_PER_ROW = 2;
 // where block b = (m, kb) of the result goes.  pack_mt == 0: canonical codes [M,K/2] / scales [M,K/16];
 // pack_mt = MT > 0: the tensor-core GEMM's activation records (gemm_tc.cu: per 256 k a record of MT*128 code bytes in
 // 8-token x 16-byte core matrices + four 512-byte scale chunks in tcgen05.cp order), `codes` = first record.
+// pack_mt < 0: the CUDA-core GEMV's own activation records at M = 1 (GEMV_XRECORD_BYTES per 32 k: the 2 x 16 E2M1 values
+// as f16 -- exact --, then the two block scales as FP32), so that the GEMV stages them with one bulk copy.
 __device__ __forceinline__ void store_block(uint8_t* codes, uint8_t* scales, int pack_mt, int b, int m, int kb, uint2 c, uint8_t s) {
-    if (pack_mt == 0) {
+    if (pack_mt < 0) {
+        uint8_t* rec = codes + (size_t)(kb >> 1) * GEMV_XRECORD_BYTES;
+        uint32_t lo[4], hi[4];
+        cvt_word_e2m1(c.x, lo);
+        cvt_word_e2m1(c.y, hi);
+        uint4* dst = reinterpret_cast<uint4*>(rec + (kb & 1) * 32);
+        dst[0] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+        dst[1] = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<float*>(rec + 64 + (kb & 1) * 4) = e4m3_to_float(s);
+    } else if (pack_mt == 0) {
         *reinterpret_cast<uint2*>(codes + (int64_t)b * 8) = c;      // [M,K/2] contiguous: block b -> 8 bytes
         scales[b] = s;
     } else {

@@ -241,3 +241,46 @@ def test_pinned_host_activations_and_outputs(B, M):
     torch.cuda.synchronize()
     assert torch.equal(xp1, xp2) and torch.equal(gx1, gx2)
     assert torch.equal(yt_dev.cpu(), yt_pin)
+
+
+# ---- quantizer -> GEMV through the GEMV's own activation records (M = 1) ------------------------------------------
+@pytest.mark.parametrize("N,K", [(2048, 2048), (300, 1296), (64, 16), (1000, 2576), (5120, 8192), (10240, 5120), (512, 25600)])
+@pytest.mark.parametrize("mode", ["dynamic", "static"])
+def test_gemv_records_equal_canonical_path(B, N, K, mode):
+    """nvfp4_quantize_act_records + nvfp4_gemv_records == nvfp4_quantize_act + nvfp4_gemv bit for bit (and so the oracle's
+    tolerance holds); ragged K (half-filled last record), K parts > 1 (small N), K slices (long rows)."""
+    wc, ws, gw = U.oracle_weight(N, K, 6, 1)
+    blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws))
+    d_gw = U.dev_f32(gw)
+    xbits = inputs.make_activation_bits(1, K, 6, 1)
+    x = U.dev_bf16_from_bits(xbits)
+    gmode = B.GSCALE_STATIC if mode == "static" else B.GSCALE_DYNAMIC
+    g_in = (lambda: U.dev_f32(0.004)) if mode == "static" else (lambda: None)
+    c, s, g = B.nvfp4_quantize_act(x, gscale=g_in(), gscale_mode=gmode)
+    y_ref = B.nvfp4_gemv(B.MODE_W4A4, blob, d_gw, N, K, c, s, g, y_dtype=B.DTYPE_F32)
+    xrec = B.nvfp4_new_xrecords(N, K, "cuda")
+    _, g2 = B.nvfp4_quantize_act_records(x, xrec, gscale=g_in(), gscale_mode=gmode)
+    y = B.nvfp4_gemv_records(blob, d_gw, N, K, xrec, g2, y_dtype=B.DTYPE_F32)
+    yb = B.nvfp4_gemv_records(blob, d_gw, N, K, xrec, g2, y_dtype=B.DTYPE_BF16)
+    torch.cuda.synchronize()
+    assert torch.equal(g, g2)
+    assert torch.equal(y, y_ref)
+    assert np.array_equal(U.host_bf16_bits(yb), orc.f32_to_bf16_bits(y.cpu().numpy()))
+    oxc, oxs, ogx = orc.quantize(orc.bf16_bits_to_f32(xbits), g=np.float32(0.004) if mode == "static" else None)
+    Y, A = orc.gemv_w4a4(wc, ws, gw, oxc, oxs, ogx)
+    U.check_gemv(U.host_y_f64(y), Y, A, f"records N={N} K={K} {mode}")
+    # a second token through the same (once zero-filled) buffer, under graph replay
+    x2 = U.dev_bf16_from_bits(inputs.make_activation_bits(1, K, 7, 1))
+    gsc = g_in() if mode == "static" else torch.zeros(1, dtype=torch.float32, device="cuda")
+    wsp = B.new_workspace(1, N, K, "cuda")
+    B.nvfp4_quantize_act_records(x2, xrec, gscale=gsc, gscale_mode=gmode); B.nvfp4_gemv_records(blob, d_gw, N, K, xrec, gsc, y=y, y_dtype=B.DTYPE_F32, workspace=wsp)
+    torch.cuda.synchronize()
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr):
+        B.nvfp4_quantize_act_records(x2, xrec, gscale=gsc, gscale_mode=gmode)
+        B.nvfp4_gemv_records(blob, d_gw, N, K, xrec, gsc, y=y, y_dtype=B.DTYPE_F32, workspace=wsp)
+    gr.replay(); gr.replay(); torch.cuda.synchronize()
+    c2, s2, g3 = B.nvfp4_quantize_act(x2, gscale=g_in(), gscale_mode=gmode)
+    assert torch.equal(y, B.nvfp4_gemv(B.MODE_W4A4, blob, d_gw, N, K, c2, s2, g3, y_dtype=B.DTYPE_F32))
+    with pytest.raises(B.Nvfp4Error):
+        B.nvfp4_gemv_records(blob, d_gw, N, K, xrec, gsc, M=2)
