@@ -370,7 +370,11 @@ class ShapeBank:
         x = torch.from_numpy(xbits.view(np.int16)).cuda().view(torch.bfloat16)
         y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
         ws = B.new_workspace(M, N, K)
-        if mode == "w4a4":
+        if mode == "w4a4rec":      # M = 1: the GEMV fed by activation records (nvfp4_quantize_act_records)
+            xrec = B.nvfp4_new_xrecords(N, K, "cuda")
+            _, gx = B.nvfp4_quantize_act_records(x, xrec)
+            call = lambda b: B.nvfp4_gemv_records(b, self.gw, N, K, xrec, gx, y=y, y_dtype=B.DTYPE_BF16, workspace=ws)
+        elif mode == "w4a4":
             xc, xs, gx = B.nvfp4_quantize_act(x)
             call = lambda b: B.nvfp4_gemv(B.MODE_W4A4, b, self.gw, N, K, xc, xs, gx, y=y, y_dtype=B.DTYPE_BF16, workspace=ws)
         else:
@@ -637,6 +641,10 @@ def run_ours(args):
                     "us": round(us44, 2), "gbs": round(nb44 / us44 / 1e3, 1), "frac": round(nb44 / us44 / 1e3 / peak, 3),
                     "w4a16_us": round(us416, 2), "w4a16_frac": round(nb416 / us416 / 1e3 / peak, 3),
                     "cublas_bf16_us": round(cub[m], 2), "copies": bank.copies}
+                if m == 1:
+                    usr = bank.time_mode(1, "w4a4rec")
+                    shape_rows[m][name]["records_us"] = round(usr, 2)
+                    shape_rows[m][name]["records_frac"] = round(nb44 / usr / 1e3 / peak, 3)
             tc = bank.time_tensor_core(TC_MS)
             for m in TC_MS:
                 nb = N * K * 9 // 16 + m * (K // 2 + K // 16) + m * N * 2
