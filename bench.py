@@ -463,7 +463,8 @@ class ShapeBank:
 def chain_ms_per_token(M, layers, peak, variants=("two_calls", "fused_quant", "tensor_core")):
     """BASELINE.json configs[4]: `layers` x {QKV, O, gate_up, down} + quantizers + SiLU*mul, distinct weights per layer,
     one CUDA graph; the best of the chain's launch variants is reported with its name.  Variants: the CUDA-core GEMV
-    with separate quantizers / with the quantizer fused into the GEMV (M = 1), and the tcgen05 GEMM path."""
+    with separate quantizers / with the quantizer fused into the GEMV (M = 1) / with the quantizers writing the GEMV's
+    activation records (M = 1), and the tcgen05 GEMM path."""
     import torch
     from paper_2606_13233_b200.chain import DecodeChain
     h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
@@ -473,7 +474,7 @@ def chain_ms_per_token(M, layers, peak, variants=("two_calls", "fused_quant", "t
         if fused and M > 1:
             continue
         ch = DecodeChain(layers=layers, M=M, fused=fused, tensor_core=label.startswith("tensor_core"),
-                         static_scales=(label == "tensor_core_static"))
+                         static_scales=(label == "tensor_core_static"), records=(label == "records"))
         ch.calibrate(h0)
         ch.step()
         torch.cuda.synchronize()
@@ -710,7 +711,7 @@ def run_ours(args):
                               "ref": "PAPER.md:570-573 Table 16, B200, another machine: context"}}
         if not args.no_chain:
             try:
-                chain = chain_ms_per_token(1, args.layers, peak, variants=("two_calls", "fused_quant"))
+                chain = chain_ms_per_token(1, args.layers, peak, variants=("two_calls", "fused_quant", "records"))
                 chain["tensor_core_m1"] = chain_ms_per_token(1, args.layers, peak, variants=("tensor_core", "tensor_core_static"))
                 chain["tensor_core_m8"] = chain_ms_per_token(8, args.layers, peak, variants=("tensor_core", "tensor_core_static"))
             except Exception as e:                                        # e.g. not enough free memory on a shared GPU
@@ -908,14 +909,15 @@ def run_chain(args):
     from paper_2606_13233_b200.chain import DecodeChain
     peak, _ = measured_peak()
     for M, fused, producer, tc in ((1, False, True, 0), (2, False, True, 0), (4, False, True, 0), (8, False, True, 0),
-                                   (1, True, True, 0), (1, False, False, 0), (1, True, False, 0),
+                                   (1, True, True, 0), (1, False, False, 0), (1, True, False, 0), (1, False, True, -1),
                                    (1, False, True, 1), (2, False, True, 1), (4, False, True, 1), (8, False, True, 1), (32, False, True, 1),
                                    (1, False, True, 2), (2, False, True, 2), (4, False, True, 2), (8, False, True, 2), (16, False, True, 2), (32, False, True, 2),
                                    (1, False, True, 3), (2, False, True, 3), (4, False, True, 3), (8, False, True, 3), (16, False, True, 3), (32, False, True, 3)):
         # tc: 0 = CUDA-core GEMV, 1 = tensor-core GEMM with quantizer launches, 2 = tensor-core GEMM, static scales, quantizers fused
         # into the GEMM epilogues (gate_up: own launch for SiLU*mul+quantize), 3 = 2 with SiLU*mul+quantize in gate_up's epilogue too
+        # tc = -1: the CUDA-core chain through the GEMV's activation records (M = 1)
         ch = DecodeChain(layers=args.layers, M=M, fused=fused, fused_producer=producer, tensor_core=tc > 0, static_scales=tc >= 2,
-                         fuse_gate_up=tc == 3)
+                         fuse_gate_up=tc == 3, records=tc == -1)
         h0 = torch.from_numpy(inputs.make_activation_bits(M, 5120, 0, 99).view(np.int16)).cuda().view(torch.bfloat16)
         ch.calibrate(h0)
         ch.step()

@@ -220,6 +220,8 @@ int nvfp4_get_layout_kparts(int N, int K);
  *                                   buffer must be ZERO-FILLED once: the quantizer writes the blocks below K only.
  *   nvfp4_quantize_act_records      x_bf16 [device] BF16 [1, K]; xrec_out [device] the records; gscale / gscale_mode as for
  *                                   nvfp4_quantize_act (NVFP4_GSCALE_DYNAMIC or _STATIC); M must be 1
+ *   nvfp4_silu_mul_quantize_records nvfp4_silu_mul_quantize writing the records (down_proj's input from gate_up's BF16 output
+ *                                   [1, 2I]; h_bf16_opt as there); M must be 1
  *   nvfp4_gemv_records              w_blob / w_gscale / y / workspace as for nvfp4_gemv (same workspace size); xrec from
  *                                   nvfp4_quantize_act_records for the same K; x_gscale [device] one float; M must be 1
  * Errors as for nvfp4_gemv; M != 1 -> NVFP4_ERR_UNSUPPORTED_SHAPE.
@@ -227,6 +229,8 @@ int nvfp4_get_layout_kparts(int N, int K);
 size_t nvfp4_gemv_xrecord_bytes(int N, int K);
 int nvfp4_quantize_act_records(const void* x_bf16, int M, int K, int64_t ldx, void* xrec_out, float* gscale, int gscale_mode,
                                void* stream);
+int nvfp4_silu_mul_quantize_records(const void* gu_bf16, int M, int I, void* xrec_out, float* gscale, int gscale_mode,
+                                    void* h_bf16_opt, void* stream);
 int nvfp4_gemv_records(const void* w_blob, const float* w_gscale, int N, int K, const void* xrec, const float* x_gscale, int M,
                        void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream);
 

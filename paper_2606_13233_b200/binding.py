@@ -33,7 +33,7 @@ SYMBOLS = ("nvfp4_version", "nvfp4_last_cuda_error", "nvfp4_quantize_act", "nvfp
            "nvfp4_gemm_packed", "nvfp4_gemm_set_config", "nvfp4_gemv_noalloc", "nvfp4_gemm_packed_quant_out",
            "nvfp4_gemm_w4a16", "nvfp4_gemm_w4a16_workspace_bytes", "nvfp4_gemm_repack_weight_gate_up",
            "nvfp4_gemm_unpack_weight_gate_up", "nvfp4_gemm_packed_silu_quant_out", "nvfp4_gemv_xrecord_bytes",
-           "nvfp4_quantize_act_records", "nvfp4_gemv_records")
+           "nvfp4_quantize_act_records", "nvfp4_gemv_records", "nvfp4_silu_mul_quantize_records")
 
 
 class Nvfp4Error(RuntimeError):
@@ -79,6 +79,8 @@ def _load():
     lib.nvfp4_gemv_xrecord_bytes.argtypes = [c_int, c_int]
     lib.nvfp4_quantize_act_records.restype = c_int
     lib.nvfp4_quantize_act_records.argtypes = [vp, c_int, c_int, c_i64, vp, vp, c_int, vp]
+    lib.nvfp4_silu_mul_quantize_records.restype = c_int
+    lib.nvfp4_silu_mul_quantize_records.argtypes = [vp, c_int, c_int, vp, vp, c_int, vp, vp]
     lib.nvfp4_gemv_records.restype = c_int
     lib.nvfp4_gemv_records.argtypes = [vp, vp, c_int, c_int, vp, vp, c_int, vp, c_int, c_i64, vp, c_sz, vp]
     lib.nvfp4_gemv_fused_quant.restype = c_int
@@ -424,6 +426,15 @@ def nvfp4_quantize_act_records(x_bf16, xrec, gscale=None, gscale_mode=GSCALE_DYN
     if gscale is None:
         gscale = torch.zeros(1, dtype=torch.float32, device=xrec.device)
     _check(lib.nvfp4_quantize_act_records(_ptr(x_bf16), M, K, x_bf16.stride(0), _ptr(xrec), _ptr(gscale), gscale_mode, _stream()))
+    return xrec, gscale
+
+
+def nvfp4_silu_mul_quantize_records(gu_bf16, xrec, gscale=None, gscale_mode=GSCALE_DYNAMIC, h=None):
+    """BF16 gate_up [1, 2I] -> records of h = silu(gate) * up for nvfp4_gemv_records (and optionally h itself)."""
+    M, I = gu_bf16.shape[0], gu_bf16.shape[1] // 2
+    if gscale is None:
+        gscale = torch.zeros(1, dtype=torch.float32, device=xrec.device)
+    _check(lib.nvfp4_silu_mul_quantize_records(_ptr(gu_bf16), M, I, _ptr(xrec), _ptr(gscale), gscale_mode, _ptr(h), _stream()))
     return xrec, gscale
 
 

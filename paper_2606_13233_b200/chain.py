@@ -21,11 +21,14 @@ QWEN3_32B_DIMS = dict(hidden=5120, qkv=10240, o_in=8192, inter=25600)
 class DecodeChain:
     def __init__(self, layers: int, M: int, dims=None, seed: int = 0, device="cuda", fused: bool = False,
                  fused_producer: bool = True, tensor_core: bool = False, static_scales: bool = False,
-                 fuse_gate_up: bool = False):
+                 fuse_gate_up: bool = False, records: bool = False):
         # static_scales (tensor-core path only; the paper's deployed flow): every projection's input global
         # scale is fixed by calibrate(), and each GEMM quantises the NEXT projection's input in its own epilogue
         # (nvfp4_gemm_packed_quant_out): 5 launches per layer -- 4 GEMMs + the SiLU*mul/quantize producer
         self.static_scales = static_scales and tensor_core
+        # records (CUDA-core path, M = 1, two calls per projection): the quantizers write the GEMV's own activation records
+        # (nvfp4_quantize_act_records / nvfp4_silu_mul_quantize_records -> nvfp4_gemv_records), bit-identical outputs
+        self.records = records and not tensor_core and not fused and fused_producer and M == 1
         # fuse_gate_up: SiLU*mul + quantize in gate_up's own epilogue (nvfp4_gemm_packed_silu_quant_out, 4 launches per layer).
         # Off by default: measured slower in the chain at every M (profiles/r02_sweep.md) -- the separate producer launch
         # hides under the down GEMM's pipeline fill, while the fused epilogue lengthens gate_up's tail (and for M > 16 its
@@ -68,6 +71,7 @@ class DecodeChain:
         self.xc = torch.empty((M, kmax // 2), dtype=u8, device=device)   # reused NVFP4 activation buffers
         self.xs = torch.empty((M, kmax // 16), dtype=u8, device=device)
         self.gx = torch.zeros(1, dtype=torch.float32, device=device)
+        self.xrec = [B.nvfp4_new_xrecords(N, K, device) for _, N, K in self.shapes] if self.records else None
         if tensor_core:
             self.ws = [B.nvfp4_gemm_packed_new_workspace(M, N, K, device) for _, N, K in self.shapes]
             self.xpack = torch.empty(B.lib.nvfp4_gemm_packed_act_bytes(M, kmax), dtype=u8, device=device)
@@ -85,6 +89,10 @@ class DecodeChain:
     def _down_from_gate_up(self, l, y, keep_h=False):
         """down projection fed by the fused producer: SiLU*mul + quantize in one launch, then the W4A4 GEMV."""
         blob, gw, N, K = self.w[l][3]
+        if self.records:
+            B.nvfp4_silu_mul_quantize_records(self.y_gu, self.xrec[3], self.gx, h=self.act if keep_h else None)
+            B.nvfp4_gemv_records(blob, gw, N, K, self.xrec[3], self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[3])
+            return
         if self.tensor_core:
             if self.M * K <= 524288:                      # the one-launch producer holds the whole [M, I] tensor in one cluster
                 B.nvfp4_silu_mul_quantize_packed(self.y_gu, self.xpack, self.gx, h_out=self.act if keep_h else None)
@@ -100,6 +108,10 @@ class DecodeChain:
 
     def _proj(self, l, i, x, y):
         blob, gw, N, K = self.w[l][i]
+        if self.records:
+            B.nvfp4_quantize_act_records(x, self.xrec[i], self.gx)
+            B.nvfp4_gemv_records(blob, gw, N, K, self.xrec[i], self.gx, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])
+            return
         if self.tensor_core:
             B.nvfp4_quantize_act_packed(x, self.xpack, self.gx)
             B.nvfp4_gemm_packed(blob, gw, N, K, self.xpack, self.gx, self.M, y=y, y_dtype=B.DTYPE_BF16, workspace=self.ws[i])

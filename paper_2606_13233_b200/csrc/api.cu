@@ -376,6 +376,20 @@ int nvfp4_quantize_act_records(const void* x_bf16, int M, int K, int64_t ldx, vo
     return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
 }
 
+int nvfp4_silu_mul_quantize_records(const void* gu_bf16, int M, int I, void* xrec_out, float* gscale, int gscale_mode,
+                                    void* h_bf16_opt, void* stream) {
+    g_last_err[0] = 0;
+    if (!gu_bf16 || !xrec_out || !gscale) return NVFP4_ERR_INVALID_ARG;
+    if (gscale_mode != NVFP4_GSCALE_DYNAMIC && gscale_mode != NVFP4_GSCALE_STATIC) return NVFP4_ERR_INVALID_ARG;
+    if (M != 1 || !shape_ok(M, 1, I)) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (gscale_mode != NVFP4_GSCALE_STATIC && (int64_t)M * I > 524288) return NVFP4_ERR_UNSUPPORTED_SHAPE;
+    if (!aligned16(gu_bf16) || !aligned16(xrec_out) || (h_bf16_opt && !aligned16(h_bf16_opt)) ||
+        (reinterpret_cast<uintptr_t>(gscale) & 3u)) return NVFP4_ERR_ALIGNMENT;
+    cudaError_t e = launch_silu_mul_quantize(gu_bf16, M, I, static_cast<uint8_t*>(xrec_out), nullptr, gscale, gscale_mode,
+                                             h_bf16_opt, static_cast<cudaStream_t>(stream), -1);
+    return e == cudaSuccess ? NVFP4_OK : cuda_fail(e);
+}
+
 int nvfp4_gemv_records(const void* w_blob, const float* w_gscale, int N, int K, const void* xrec, const float* x_gscale, int M,
                        void* y, int y_dtype, int64_t ldy, void* workspace, size_t ws_bytes, void* stream) {
     g_last_err[0] = 0;

@@ -42,6 +42,17 @@ def test_chain_small_dims_every_stage(M, fused, producer):
     h0 = U.dev_bf16_from_bits(inputs.make_activation_bits(M, 256, 0, 77))
     ch.set_input(h0); ch.step(); torch.cuda.synchronize()
     ref = ch.h.clone()
+    if M == 1 and not fused and producer:
+        # the same chain through the GEMV's activation records (nvfp4_*_records): same bits at every stage
+        ch2 = DecodeChain(layers=3, M=M, dims=dims, seed=5, records=True)
+        assert ch2.records
+        ch2.calibrate(h0)
+        taps2 = []
+        ch2.step(taps2)
+        torch.cuda.synchronize()
+        for (l, name, x, y), (l2, name2, x2, y2) in zip(taps, taps2):
+            assert (l, name) == (l2, name2) and torch.equal(x, x2) and torch.equal(y, y2), (l, name)
+        assert torch.equal(ch2.h, ref)
     g = torch.cuda.CUDAGraph()
     ch.set_input(h0)
     with torch.cuda.graph(g):

@@ -284,3 +284,20 @@ def test_gemv_records_equal_canonical_path(B, N, K, mode):
     assert torch.equal(y, B.nvfp4_gemv(B.MODE_W4A4, blob, d_gw, N, K, c2, s2, g3, y_dtype=B.DTYPE_F32))
     with pytest.raises(B.Nvfp4Error):
         B.nvfp4_gemv_records(blob, d_gw, N, K, xrec, gsc, M=2)
+
+
+def test_silu_mul_quantize_records_equals_two_kernels(B):
+    """nvfp4_silu_mul_quantize_records + nvfp4_gemv_records == nvfp4_silu_mul_quantize + nvfp4_gemv bit for bit (down_proj shape)"""
+    I, N = 25600, 256
+    rng = np.random.default_rng(11)
+    gu = U.dev_bf16_from_bits(orc.f32_to_bf16_bits((rng.standard_normal((1, 2 * I)) * 2.0).astype(np.float32)))
+    wc, ws, gw = U.oracle_weight(N, I, 8, 1)
+    blob = B.nvfp4_repack_weight(U.dev_u8(wc), U.dev_u8(ws)); d_gw = U.dev_f32(gw)
+    h1 = torch.empty((1, I), dtype=torch.bfloat16, device="cuda"); h2 = torch.empty_like(h1)
+    c, s, g = B.nvfp4_silu_mul_quantize(gu, h=h1)
+    y_ref = B.nvfp4_gemv(B.MODE_W4A4, blob, d_gw, N, I, c, s, g, y_dtype=B.DTYPE_F32)
+    xrec = B.nvfp4_new_xrecords(N, I, "cuda")
+    _, g2 = B.nvfp4_silu_mul_quantize_records(gu, xrec, h=h2)
+    y = B.nvfp4_gemv_records(blob, d_gw, N, I, xrec, g2, y_dtype=B.DTYPE_F32)
+    torch.cuda.synchronize()
+    assert torch.equal(g, g2) and torch.equal(h1, h2) and torch.equal(y, y_ref)
